@@ -1,0 +1,241 @@
+/*
+ * fsw.h -- C ABI of the B200-native fisheye plane-sweeping stereo library (libfsw.so).
+ *
+ * What it computes: the depth-map estimation stage of arXiv 1809.06132
+ * ("Real-time dense mapping for self-driving vehicles using fisheye cameras"),
+ * PAPER.md section III-A (lines 69-99): plane-sweeping stereo run directly on
+ * the fisheye images through the unified projective camera model (PAPER.md:149,
+ * back-projection = Eq. 1), ZNCC matching cost over a w x w
+ * window, accumulation over >2 cameras, best depth
+ * candidate with first / second best cost, the best-cost and
+ * uniqueness-ratio filters, the two-scale strategy
+ * and the dynamic-object mask.  Readings of passages the paper
+ * leaves open are listed in DESIGN.md.
+ *
+ * Conventions
+ *  - Camera frame: x right, y down, z forward.  Pixel centres at integer
+ *    coordinates: I(u,v) for integer u,v is the stored sample; u in [0,W-1].
+ *  - Extrinsics are rig->camera: X_cam = R * X_rig + t (R row-major).
+ *  - All functions return an int32 status (FSW_OK = 0, negative = error) and
+ *    never throw.  fsw_last_error() returns a thread-local message for the last
+ *    failing call of the calling thread.
+ *  - Geometric failures (pixel outside the field of view, ray parallel to a
+ *    plane, projection outside a view image) are VALUES, not errors: they make a
+ *    view / plane / pixel invalid.  An invalid depth is exactly 0.0f.
+ *  - Every struct starts with `struct_size` (= sizeof the struct as compiled by
+ *    the caller) so the ABI can grow.
+ *  - "device" pointers are CUDA device memory of the context's device; "host"
+ *    pointers are ordinary process memory.  The library never takes ownership of
+ *    a caller buffer.
+ *  - There is no CPU fallback: without a CUDA device fsw_context_create fails
+ *    with FSW_E_CUDA.
+ */
+#ifndef FSW_H
+#define FSW_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define FSW_VERSION_MAJOR 0
+#define FSW_VERSION_MINOR 1
+
+/* status codes */
+#define FSW_OK 0
+#define FSW_E_INVALID_ARG (-1) /* null pointer, bad size, bad enum, struct_size mismatch */
+#define FSW_E_CONFIG (-2)      /* arguments are well-formed but describe an impossible rig / plane set */
+#define FSW_E_CUDA (-3)        /* a CUDA runtime call failed (message holds cudaGetErrorString) */
+#define FSW_E_NOMEM (-4)
+#define FSW_E_UNSUPPORTED (-5)
+
+/* limits */
+#define FSW_MAX_CAMERAS 8
+#define FSW_MAX_PLANES 1024
+#define FSW_MAX_FAMILIES 8
+#define FSW_MAX_WINDOW 15
+
+/* pixel types of input images */
+#define FSW_U8 0  /* uint8 grey levels 0..255 ("gray scale images") */
+#define FSW_F32 1 /* float32 intensities, any scale */
+
+/* plane spacing inside a family */
+#define FSW_INVERSE 0 /* uniform in 1/d */
+#define FSW_LINEAR 1  /* uniform in d   */
+
+/* filters_enabled bits */
+#define FSW_FILTER_COST 1  /* invalidate if best cost > alpha(row)            */
+#define FSW_FILTER_RATIO 2 /* invalidate if second best < beta * max(best,1e-6) */
+
+/* depth_kind */
+#define FSW_DEPTH_RANGE 0 /* Euclidean range along the unit ray (PAPER.md:161-162 integrates along the ray) */
+#define FSW_DEPTH_Z 1     /* range * r_z */
+
+/* reason codes written to fsw_depth_out.valid_reason (0 = valid) */
+#define FSW_REASON_OK 0
+#define FSW_REASON_NO_PLANE 1     /* no plane has a finite cost (outside FOV / ROI / every view invalid) */
+#define FSW_REASON_COST_FILTER 2
+#define FSW_REASON_RATIO_FILTER 3
+#define FSW_REASON_MASKED 4
+
+/* bit set in plane_index where the full-resolution crop pass supplied the value (multi-resolution call) */
+#define FSW_INDEX_FROM_CROP (1 << 14)
+
+typedef struct fsw_rig fsw_rig;
+typedef struct fsw_planeset fsw_planeset;
+typedef struct fsw_context fsw_context;
+
+/* One fisheye camera: unified projective (Mei) model.
+ * projection: X -> X/|X| on the unit sphere -> m = (X_x, X_y) / (X_z + xi |X|)
+ *             -> m_d = m (1 + k1 r^2 + k2 r^4) + tangential(p1,p2), r^2 = |m|^2
+ *             -> (u,v) = (fx m_d.x + cx, fy m_d.y + cy);
+ * back-projection: undistort, then Eq. 1.  Rays / points further than
+ * fov_max_deg/2 from the optical axis are outside the camera (invalid). */
+typedef struct fsw_camera {
+    uint32_t struct_size;
+    int32_t width, height;
+    double fx, fy, cx, cy;
+    double xi;             /* mirror parameter, 0 <= xi <= 3 */
+    double k1, k2, p1, p2; /* distortion on the normalised plane (0 = none) */
+    double fov_max_deg;    /* full field of view in degrees, (0, 360] */
+    double R[9];           /* rig->camera rotation, row-major, orthonormal within 1e-5 */
+    double t[3];           /* rig->camera translation, metres */
+} fsw_camera;
+
+/* One family of sweep planes n.X = d_k in the REFERENCE-camera frame (PAPER.md:74:
+ * fronto-parallel to the reference image plane, and parallel to the ground).
+ * Plane k (0 <= k < n_planes): s_k = s_first + k (s_last - s_first)/(n_planes-1),
+ * s = 1/d (FSW_INVERSE) or d (FSW_LINEAR).  Global plane index = families
+ * concatenated in call order. */
+typedef struct fsw_plane_family {
+    uint32_t struct_size;
+    double normal[3]; /* need not be unit length; normalised by the library */
+    int32_t n_planes; /* >= 1 */
+    int32_t spacing;  /* FSW_INVERSE / FSW_LINEAR */
+    double d_first, d_last; /* metres; > 0 */
+} fsw_plane_family;
+
+typedef struct fsw_rect {
+    int32_t x0, y0, w, h;
+} fsw_rect;
+
+typedef struct fsw_sweep_params {
+    uint32_t struct_size;
+    int32_t window;          /* odd, 3..FSW_MAX_WINDOW: side of the ZNCC window (9 full-res, 7 half-res) */
+    int32_t subpixel;        /* 1 = three-point parabola over the plane index in the spacing variable */
+    int32_t filters_enabled; /* FSW_FILTER_* bits */
+    int32_t depth_kind;      /* FSW_DEPTH_RANGE / FSW_DEPTH_Z */
+    fsw_rect roi;            /* output region on the reference raster; w <= 0 or h <= 0 = whole image */
+    int32_t horizon_row;     /* rows < horizon_row use alpha_upper, others alpha_lower (0.05 / 0.3) */
+    float alpha_upper, alpha_lower;
+    float beta;      /* keep iff second >= beta * max(best, 1e-6) */
+    float var_floor; /* floor of sqrt(var_a var_b) in the ZNCC denominator, in intensity units squared */
+    float range_max; /* a ray/plane intersection further than this (metres along the ray) is invalid */
+    float* debug_cost_volume; /* device, nullable: [P][H][W] float32, view-averaged cost, +inf = undefined */
+} fsw_sweep_params;
+
+/* one input image: row-major, pitch in BYTES */
+typedef struct fsw_image {
+    const void* data; /* device pointer (host pointer for fsw_compute_depth*_host) */
+    size_t pitch_bytes;
+    int32_t dtype; /* FSW_U8 / FSW_F32 */
+} fsw_image;
+
+/* output maps, all at the reference camera's full resolution, row-major, pitches in BYTES.
+ * depth is required; every other pointer may be NULL. */
+typedef struct fsw_depth_out {
+    uint32_t struct_size;
+    float* depth;        size_t depth_pitch;        /* metres, 0.0f = invalid */
+    float* best_cost;    size_t best_cost_pitch;    /* c1, +inf where no plane */
+    float* second_cost;  size_t second_cost_pitch;  /* c2 (non-adjacent second best), +inf where no plane */
+    int16_t* plane_index; size_t plane_index_pitch; /* winning global plane index, -1 where no plane */
+    uint8_t* valid_reason; size_t valid_reason_pitch; /* FSW_REASON_* */
+} fsw_depth_out;
+
+typedef struct fsw_counters {
+    uint32_t struct_size;
+    int64_t n_eval;      /* (pixel, plane, view) triples with a finite matching cost in the last call */
+    int64_t n_raw_valid; /* pixels with at least one finite plane cost (before filters / mask) */
+    int64_t n_valid;     /* pixels valid after filters and mask */
+    int64_t n_launches;  /* CUDA kernels launched by the last call */
+} fsw_counters;
+
+/* ---- version / errors ---------------------------------------------------- */
+int32_t fsw_version(int32_t* major, int32_t* minor);
+const char* fsw_last_error(void);
+
+/* ---- rig (host-only, no CUDA needed) ------------------------------------- */
+/* cams: host array of n_cams cameras (copied).  2 <= n_cams <= FSW_MAX_CAMERAS; ref_index selects the reference
+ * camera; every other camera is a matching view, used in array order.
+ * Errors: FSW_E_INVALID_ARG (null, n_cams, ref_index, struct_size), FSW_E_CONFIG (fx,fy <= 0; principal point outside
+ * the image; R not orthonormal; xi outside [0,3]; fov outside (0,360]; distortion not invertible inside the FOV). */
+int32_t fsw_rig_create(const fsw_camera* cams, int32_t n_cams, int32_t ref_index, fsw_rig** out);
+int32_t fsw_rig_destroy(fsw_rig* rig);
+/* relative pose reference -> camera `cam`: X_cam = R X_ref + T (R row-major, 9 doubles; T 3 doubles) */
+int32_t fsw_rig_relative_pose(const fsw_rig* rig, int32_t cam, double* R, double* T);
+/* a rig-frame direction (e.g. "down" = (0,1,0)) expressed in the reference-camera frame (the ground
+ * plane normal comes from the extrinsic calibration) */
+int32_t fsw_ground_normal_in_ref(const fsw_rig* rig, const double* dir_rig, double* out);
+
+/* ---- plane set (host-only) ------------------------------------------------ */
+/* Errors: FSW_E_INVALID_ARG (null, n_fams outside 1..FSW_MAX_FAMILIES, spacing enum), FSW_E_CONFIG (n_planes < 1,
+ * d <= 0, zero normal, total planes > FSW_MAX_PLANES). */
+int32_t fsw_planeset_create(const fsw_plane_family* fams, int32_t n_fams, fsw_planeset** out);
+int32_t fsw_planeset_destroy(fsw_planeset* ps);
+int32_t fsw_planeset_size(const fsw_planeset* ps, int32_t* n_planes);
+/* copies out the plane table: s[k] spacing variable, d[k] offset, family[k]; any pointer may be NULL */
+int32_t fsw_planeset_table(const fsw_planeset* ps, double* s, double* d, int32_t* family);
+
+/* ---- context (needs a CUDA device) ---------------------------------------- */
+/* Owns device-side scratch (footprint-packed view images, half-resolution images and maps, counters).  Scratch is
+ * allocated lazily and reused; no hidden streams: all work is enqueued on the stream given to each call. */
+int32_t fsw_context_create(const fsw_rig* rig, int32_t cuda_device, fsw_context** out);
+int32_t fsw_context_destroy(fsw_context* ctx);
+
+/* ---- depth for one synchronized frame set ------------------- */
+/* images: host array of n_cams fsw_image descriptors in rig order, each `data` a DEVICE pointer to an image of that
+ * camera's width x height.  mask: device, nullable, uint8 [H][W] of the reference camera, non-zero = invalidate
+ * (PAPER.md:66).  out: device output maps.  Asynchronous: work is enqueued on cuda_stream (a cudaStream_t; NULL =
+ * default stream) and the call returns; the caller keeps every buffer alive until the stream reaches this work.
+ * Errors: FSW_E_INVALID_ARG (nulls, window even / out of range, pitches too small, dtype enum),
+ * FSW_E_CUDA (launch or allocation failure). */
+int32_t fsw_compute_depth(fsw_context* ctx, const fsw_planeset* planes, const fsw_sweep_params* params,
+                          const fsw_image* images, const uint8_t* mask, size_t mask_pitch,
+                          const fsw_depth_out* out, void* cuda_stream);
+
+/* Two-scale strategy of PAPER.md:88-90: every image is 2x2-box downsampled and swept over the whole field of view
+ * with planes_low / params_low (intrinsics f/2, c' = (c-0.5)/2); the result is upsampled (nearest neighbour); the
+ * full-resolution images are swept inside `crop` with planes_crop / params_crop; inside the crop the full-resolution
+ * estimate wins where it has any finite plane cost, elsewhere the upsampled one is used; then the filters (thresholds
+ * of params_crop) and the mask.  plane_index carries FSW_INDEX_FROM_CROP where the crop pass supplied the value. */
+int32_t fsw_compute_depth_multires(fsw_context* ctx, const fsw_planeset* planes_low, const fsw_planeset* planes_crop,
+                                   const fsw_sweep_params* params_low, const fsw_sweep_params* params_crop,
+                                   fsw_rect crop, const fsw_image* images, const uint8_t* mask, size_t mask_pitch,
+                                   const fsw_depth_out* out, void* cuda_stream);
+
+/* Same two calls with HOST buffers: images[i].data, mask and every pointer of `out` are host memory (pinned memory
+ * makes the copies asynchronous).  The library stages them through context-owned device buffers on cuda_stream:
+ * host->device copies, the kernels, device->host copies, then synchronizes the stream before returning. */
+int32_t fsw_compute_depth_host(fsw_context* ctx, const fsw_planeset* planes, const fsw_sweep_params* params,
+                               const fsw_image* images, const uint8_t* mask, size_t mask_pitch,
+                               const fsw_depth_out* out, void* cuda_stream);
+int32_t fsw_compute_depth_multires_host(fsw_context* ctx, const fsw_planeset* planes_low,
+                                        const fsw_planeset* planes_crop, const fsw_sweep_params* params_low,
+                                        const fsw_sweep_params* params_crop, fsw_rect crop, const fsw_image* images,
+                                        const uint8_t* mask, size_t mask_pitch, const fsw_depth_out* out,
+                                        void* cuda_stream);
+
+/* Counters of the most recent compute call on this context.  Synchronizes the stream that call used. */
+int32_t fsw_get_last_counters(fsw_context* ctx, fsw_counters* out);
+
+/* ---- measurement helper ---------------------------------------------------- */
+/* Runs a dependent-FFMA-chain kernel on `cuda_stream` and reports the FP32 throughput it reached (TFLOP/s, counting
+ * an FMA as 2) and the kernel time.  Used by bench.py for the "alu" roofline denominator. Synchronizes. */
+int32_t fsw_measure_fp32_peak(int32_t cuda_device, void* cuda_stream, double* tflops, double* ms);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FSW_H */
