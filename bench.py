@@ -1,0 +1,355 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the fisheye plane-sweep hot path on B200 (one JSON line on stdout).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C5|C3] [--impl ours|reference]
+
+A "step" is one pass of the whole hot path (footprint pack + fused sweep S1..S12) over one synchronized
+frame set of the workload: BASELINE.json configs[4] (C5, the throughput stream: config-3 rig moving 0.5 m per frame,
+192 fronto + 64 ground planes, 9x9 ZNCC, filters and masks on) by default, or configs[2] (C3) with --workload C3.
+`value` = finite (pixel, plane, view) cost evaluations per second, inputs resident in HBM; `e2e` = the same through
+fsw_compute_depth_host (pinned host buffers, copies inside the timed region).  N > 1 (torchrun): frame sets are
+independent, so each rank runs the same number of steps on its own frames -- no data-path collective, "weak".
+--impl reference times the CPU oracle (oracle/) on a bounded crop of the same workload, rank 0 only.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+FLOP_PER_EVAL = 70.0   # algorithmic FP32 work of one (pixel, plane, view) cost evaluation
+N_STAGED = 32          # distinct frame sets resident on the device (the C5 stream length)
+METRIC = "plane-sweep cost evals/sec (pixel x plane x view)"
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=128)
+    ap.add_argument("--warmup", type=int, default=8)
+    ap.add_argument("--workload", default="C5", choices=["C5", "C3"])
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--cpu-baseline-seconds", type=float, default=12.0)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    return ap.parse_args()
+
+
+def workload_config(name):
+    import synth
+    cfg = synth.make_config(5 if name == "C5" else 3)
+    if name == "C3":  # the C3 scene, but as a stream of N_STAGED frame sets like C5 so that inputs exceed L2
+        cfg = dict(cfg, n_frames=N_STAGED, step_m=0.5, mask_seed=None)
+    return cfg
+
+
+def workload_label(name):
+    return ("BASELINE.json configs[4]: 32-frame stream, 3 fisheye cams 1280x1024 u8, 192 fronto + 64 ground planes, "
+            "9x9 ZNCC, filters + masks" if name == "C5" else
+            "BASELINE.json configs[2]: 3 fisheye cams 1280x1024 u8, 96 fronto + 32 ground planes, 9x9 ZNCC, filters")
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons through NVML while the timed region runs."""
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.samples, self.reasons, self.stop_flag, self.max_mhz = index, [], set(), False, None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+        except Exception:
+            self.nv = None
+
+    def run(self):
+        if self.nv is None:
+            return
+        nv = self.nv
+        names = {"hw_slowdown": getattr(nv, "nvmlClocksThrottleReasonHwSlowdown", 0x8),
+                 "hw_thermal_slowdown": getattr(nv, "nvmlClocksThrottleReasonHwThermalSlowdown", 0x40),
+                 "sw_thermal_slowdown": getattr(nv, "nvmlClocksThrottleReasonSwThermalSlowdown", 0x20),
+                 "sw_power_cap": getattr(nv, "nvmlClocksThrottleReasonSwPowerCap", 0x4)}
+        while not self.stop_flag:
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for k, bit in names.items():
+                    if r & bit:
+                        self.reasons.add(k)
+            except Exception:
+                pass
+            time.sleep(0.005)
+
+    def summary(self):
+        med = float(np.median(self.samples)) if self.samples else None
+        return {"sm_mhz": med, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+def physical_gpu_index(local_rank):
+    vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+    if vis:
+        try:
+            return int(vis.split(",")[local_rank])
+        except Exception:
+            return local_rank
+    return local_rank
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+def cropped_rig(cfg, crop_w, crop_h):
+    """The workload's rig restricted to a centred crop_w x crop_h window of every camera (principal point shifted):
+    a bounded sample of the same workload for the CPU legs."""
+    cams = []
+    W, H = cfg["cams"][0]["width"], cfg["cams"][0]["height"]
+    x0, y0 = (W - crop_w) // 2, (H - crop_h) // 2
+    for c in cfg["cams"]:
+        c2 = dict(c)
+        c2.update(width=crop_w, height=crop_h, cx=c["cx"] - x0, cy=c["cy"] - y0)
+        cams.append(c2)
+    return cams, (x0, y0)
+
+
+def oracle_sample(cfg, frame_images, mask, crop_w, crop_h):
+    """Runs the oracle as it stands on a centred crop; returns (seconds, n_eval)."""
+    import oracle
+    cams, (x0, y0) = cropped_rig(cfg, crop_w, crop_h)
+    imgs = [np.ascontiguousarray(im[y0:y0 + crop_h, x0:x0 + crop_w]) for im in frame_images]
+    m = None if mask is None else np.ascontiguousarray(mask[y0:y0 + crop_h, x0:x0 + crop_w])
+    params = dict(cfg["params"], horizon_row=cfg["params"]["horizon_row"] - y0)
+    t0 = time.perf_counter()
+    out = oracle.compute_depth(cams, cfg["ref_index"], cfg["families"], params, imgs, m)
+    return time.perf_counter() - t0, int(out["n_eval"])
+
+
+def run_reference(args, rank):
+    """--impl reference: the oracle, unmodified, on the host cores; each step = one cropped frame set."""
+    if rank != 0:
+        return
+    import oracle
+    import synth
+    cfg = workload_config(args.workload)
+    oracle.build()
+    total_steps = args.steps + args.warmup
+    # size the crop so that the whole run stays within a few minutes (oracle ~ 1e7 evals/s per 8 cores)
+    budget_s = 150.0
+    planes_views = sum(f["n_planes"] for f in cfg["families"]) * (len(cfg["cams"]) - 1)
+    est_rate = 1.2e6 * max(oracle.num_threads(), 1)
+    px = max(48 * 36, int(budget_s / max(total_steps, 1) * est_rate / planes_views))
+    crop_h = int(min(640, max(36, (px / (4.0 / 3.0)) ** 0.5))) // 4 * 4
+    crop_w = int(min(848, crop_h * 4 // 3)) // 4 * 4
+    frames = {}
+    times, evals = [], []
+    for s in range(total_steps):
+        f = s % N_STAGED
+        if f not in frames:
+            frames[f] = synth.render_frame(cfg, f)
+        mask = None if cfg.get("mask_seed") is None else synth.make_mask(1280, 1024, cfg["mask_seed"] + f)
+        dt, ne = oracle_sample(cfg, frames[f], mask, crop_w, crop_h)
+        if s >= args.warmup:
+            times.append(dt)
+            evals.append(ne)
+    total = float(sum(times))
+    value = float(sum(evals)) / total if total > 0 else 0.0
+    sample = "centred %dx%d crop of each frame set (principal point shifted), all planes and views" % (crop_w, crop_h)
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": "evals/s", "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * total / max(len(times), 1),
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": workload_label(args.workload), "sample": sample},
+        "cpu_baseline": {"value": value, "unit": "evals/s", "cores": oracle.num_threads(), "kind": "oracle",
+                         "sample": sample},
+        "e2e": {"value": value, "unit": "evals/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+def run_ours(args, rank, local_rank, world):
+    import torch
+    import synth
+    import paper_1809_06132_b200 as fsw
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the hot path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    dev = torch.device("cuda", local_rank)
+    cfg = workload_config(args.workload)
+    W, H = cfg["cams"][0]["width"], cfg["cams"][0]["height"]
+
+    # ---- inputs: N_STAGED distinct frame sets per rank, resident on the device (and pinned on the host for e2e) ----
+    frame0 = rank * N_STAGED
+    host_frames, host_masks = [], []
+    for f in range(N_STAGED):
+        host_frames.append(synth.render_frame(cfg, frame0 + f))
+        if cfg.get("mask_seed") is not None:
+            host_masks.append(synth.make_mask(W, H, cfg["mask_seed"] + frame0 + f))
+    dev_frames = [[torch.from_numpy(im).to(dev) for im in fr] for fr in host_frames]
+    dev_masks = [torch.from_numpy(m).to(dev) for m in host_masks] or [None] * N_STAGED
+    rig = fsw.Rig(cfg["cams"], cfg["ref_index"])
+    planes = fsw.PlaneSet(cfg["families"])
+    ctx = fsw.Context(rig, local_rank)
+    # every frame set gets its own output maps so that the bytes touched per pass exceed the 126 MB L2
+    outs = [dict(depth=torch.empty((H, W), dtype=torch.float32, device=dev),
+                 best_cost=torch.empty((H, W), dtype=torch.float32, device=dev),
+                 second_cost=torch.empty((H, W), dtype=torch.float32, device=dev),
+                 plane_index=torch.empty((H, W), dtype=torch.int16, device=dev),
+                 valid_reason=torch.empty((H, W), dtype=torch.uint8, device=dev)) for _ in range(N_STAGED)]
+
+    def step(i):
+        f = i % N_STAGED
+        ctx.compute_depth(planes, cfg["params"], dev_frames[f], dev_masks[f], out=outs[f])
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident timing ------------------------------------------------------------------------------------
+    for i in range(args.warmup):
+        step(i)
+    torch.cuda.synchronize()
+    n_eval_step = []
+    launches = 0
+    for f in range(min(N_STAGED, args.steps)):   # per-frame N_eval from the kernel's counter (untimed pass)
+        step(f)
+        c = ctx.last_counters()
+        n_eval_step.append(c["n_eval"])
+        launches_per_step = c["n_launches"]
+    sampler = ClockSampler(physical_gpu_index(local_rank))
+    stream = torch.cuda.current_stream()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    sampler.start()
+    ev0.record(stream)
+    for i in range(args.steps):
+        step(i)
+    ev1.record(stream)
+    torch.cuda.synchronize()
+    sampler.stop_flag = True
+    barrier()
+    ms_total = ev0.elapsed_time(ev1)
+    launches = launches_per_step * args.steps
+    evals_total = float(sum(n_eval_step[i % len(n_eval_step)] for i in range(args.steps)))
+
+    # ---- the sweep kernel alone: CUDA events around its launches on the same stream (fsw_context_set_timing) ------
+    ctx.set_timing(True)
+    sweep_ms = []
+    for i in range(min(args.steps, 2 * N_STAGED)):
+        step(i)
+        sweep_ms.append(ctx.last_counters()["sweep_ms"])
+    ctx.set_timing(False)
+    sweep_ms_avg = float(np.mean(sweep_ms))
+    evals_per_launch = float(np.mean([n_eval_step[i % len(n_eval_step)] for i in range(len(sweep_ms))]))
+
+    # ---- end to end: host buffers through fsw_compute_depth_host ---------------------------------------------------
+    pin_frames = [[torch.from_numpy(im).pin_memory() for im in fr] for fr in host_frames]
+    pin_masks = [torch.from_numpy(m).pin_memory() for m in host_masks] or [None] * N_STAGED
+    pin_out = dict(depth=torch.empty((H, W), dtype=torch.float32).pin_memory())
+    h2d = sum(int(t.numel() * t.element_size()) for t in pin_frames[0]) + (W * H if host_masks else 0)
+    d2h = W * H * 4
+
+    def step_e2e(i):
+        f = i % N_STAGED
+        ctx.compute_depth(planes, cfg["params"], pin_frames[f], pin_masks[f], host=True, out=pin_out)
+
+    for i in range(3):
+        step_e2e(i)
+    e2e_steps = args.steps
+    barrier()
+    ev0.record(stream)
+    for i in range(e2e_steps):
+        step_e2e(i)
+    ev1.record(stream)
+    torch.cuda.synchronize()
+    barrier()
+    ms_e2e = ev0.elapsed_time(ev1)
+    launches += launches_per_step * e2e_steps
+
+    # ---- max over ranks ----------------------------------------------------------------------------------------------
+    t = torch.tensor([ms_total, ms_e2e], dtype=torch.float64, device=dev)
+    ev = torch.tensor([evals_total], dtype=torch.float64, device=dev)
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dist.all_reduce(ev, op=dist.ReduceOp.SUM)
+    ms_total, ms_e2e = float(t[0]), float(t[1])
+    evals_all = float(ev[0])
+
+    if rank == 0:
+        fp32_tflops, _ = fsw.measure_fp32_peak(local_rank)
+        value = evals_all / (ms_total * 1e-3)
+        e2e_value = evals_all / (ms_e2e * 1e-3)
+        achieved = evals_per_launch * FLOP_PER_EVAL / (sweep_ms_avg * 1e-3) / 1e12
+        line = {
+            "metric": METRIC, "value": value, "unit": "evals/s", "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": workload_label(args.workload), "frames_staged_per_gpu": N_STAGED,
+                       "n_eval_per_step": evals_total / args.steps, "n_nominal_per_step": W * H * planes.n_planes * (rig.n_cams - 1),
+                       "l2": "inputs and outputs rotate over %d distinct frame sets (%.0f MB per pass) > 126 MB L2" % (
+                           N_STAGED, N_STAGED * (3 * W * H + W * H + W * H * 15 + 2 * W * H * 4) / 1e6),
+                       "parallelism": "frame sets sharded over %d GPU(s), no collective" % world},
+            "depth_maps_per_s": world * args.steps / (ms_total * 1e-3) if dist is None else None,
+            "clocks": sampler.summary(),
+            "e2e": {"value": e2e_value, "unit": "evals/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                    "ms_per_step": ms_e2e / e2e_steps, "depth_maps_per_s": world * e2e_steps / (ms_e2e * 1e-3)},
+            "gpu_launches": launches,
+            "roofline": {"bound": "alu", "achieved": achieved, "peak": fp32_tflops, "unit": "TFLOP/s",
+                         "frac": achieved / fp32_tflops if fp32_tflops else None, "traffic": None,
+                         "kernel": "fsw::sweep_kernel<9,...>", "kernel_ms": sweep_ms_avg,
+                         "flop_per_eval": FLOP_PER_EVAL,
+                         "peak_source": "FFMA-chain kernel measured in this run (MEASURED_PEAKS.json has no FP32 figure); "
+                                        "nominal 148 SM x 128 lanes x 2 x clock"},
+        }
+        line["depth_maps_per_s"] = world * args.steps / (ms_total * 1e-3)
+        if not args.no_cpu_baseline:
+            line["cpu_baseline"] = cpu_baseline(cfg, host_frames[0], host_masks[0] if host_masks else None,
+                                                args.cpu_baseline_seconds)
+        print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+def cpu_baseline(cfg, frame, mask, seconds):
+    """The oracle as it stands, timed on this box's host cores on a bounded sample of the workload."""
+    import oracle
+    oracle.build()
+    cores = oracle.num_threads()
+    planes_views = sum(f["n_planes"] for f in cfg["families"]) * (len(cfg["cams"]) - 1)
+    px = seconds * 1.2e6 * cores / planes_views
+    crop_h = int(min(640, max(64, (px * 0.75) ** 0.5))) // 4 * 4
+    crop_w = int(min(848, crop_h * 4 // 3)) // 4 * 4
+    dt, ne = oracle_sample(cfg, frame, mask, crop_w, crop_h)
+    return {"value": ne / dt, "unit": "evals/s", "cores": cores, "kind": "oracle", "seconds": dt,
+            "sample": "frame set 0, centred %dx%d crop (principal point shifted), all planes and views" % (crop_w, crop_h)}
+
+
+def main():
+    args = parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.impl == "reference":
+        run_reference(args, rank)
+        return
+    run_ours(args, rank, local_rank, world)
+
+
+if __name__ == "__main__":
+    main()

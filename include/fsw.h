@@ -160,6 +160,8 @@ typedef struct fsw_counters {
     int64_t n_raw_valid; /* pixels with at least one finite plane cost (before filters / mask) */
     int64_t n_valid;     /* pixels valid after filters and mask */
     int64_t n_launches;  /* CUDA kernels launched by the last call */
+    double sweep_ms;     /* device time of the sweep kernel(s) of the last call, CUDA events on the call's stream;
+                            -1 unless fsw_context_set_timing(ctx, 1) was in effect */
 } fsw_counters;
 
 /* ---- version / errors ---------------------------------------------------- */
@@ -226,6 +228,11 @@ int32_t fsw_compute_depth_multires_host(fsw_context* ctx, const fsw_planeset* pl
                                         const fsw_sweep_params* params_crop, fsw_rect crop, const fsw_image* images,
                                         const uint8_t* mask, size_t mask_pitch, const fsw_depth_out* out,
                                         void* cuda_stream);
+
+/* on != 0: every following compute call brackets its sweep kernel launches (the dominant kernels, S1-S12) with a
+ * pair of CUDA events on the call's stream so that fsw_get_last_counters can report their device time.  Off by
+ * default (two event records per call). */
+int32_t fsw_context_set_timing(fsw_context* ctx, int32_t on);
 
 /* Counters of the most recent compute call on this context.  Synchronizes the stream that call used. */
 int32_t fsw_get_last_counters(fsw_context* ctx, fsw_counters* out);

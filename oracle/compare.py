@@ -17,7 +17,24 @@ COST_TOL = 1e-4
 DEPTH_RTOL = 1e-3
 
 
-def compare_maps(orc: dict, test: dict, cost_volumes=None, index_flag_mask: int = 0x3FFF) -> dict:
+def depth_conditioning(orc: dict, plane_s, pden=None, kbest=None) -> np.ndarray:
+    """(|ds|/s) / pden per pixel: how strongly an error of the three costs around the minimum moves the refined
+    depth.  With |error| <= eps on each cost, |d delta| <= 3 eps / pden, and d depth / depth = d delta * |ds| / s
+    ("Tolerances").  inf where the parabola was not applied is replaced by 0 (no refinement -> no
+    sensitivity)."""
+    k = (orc["kbest"] if kbest is None else kbest).astype(np.int64)
+    pd = orc["pden"] if pden is None else pden
+    plane_s = np.asarray(plane_s, dtype=np.float64)
+    ks = np.clip(k & 0x3FFF, 0, len(plane_s) - 1)
+    kn = np.clip(ks + 1, 0, len(plane_s) - 1)
+    ds = np.abs(plane_s[kn] - plane_s[ks])
+    s = plane_s[ks]
+    with np.errstate(divide="ignore", invalid="ignore"):
+        cond = np.where(pd > 0, (ds / s) / pd, 0.0)
+    return np.where(k >= 0, cond, 0.0)
+
+
+def compare_maps(orc: dict, test: dict, cost_volumes=None, index_flag_mask: int = 0x3FFF, depth_cond=None) -> dict:
     """orc: dict from oracle.compute_depth / compute_depth_multires (float64 maps, 'reason', 'kbest', 'c2raw' ...).
     test: dict of numpy arrays depth, best_cost, second_cost, plane_index, valid_reason.
     cost_volumes: oracle cost volume [P,H,W] (single pass), or a pair (cost_lo at half resolution, cost_hi) for the
@@ -73,6 +90,11 @@ def compare_maps(orc: dict, test: dict, cost_volumes=None, index_flag_mask: int 
         ddepth = np.abs(np.asarray(test["depth"], dtype=np.float64) - orc["depth"]) / np.maximum(orc["depth"], 1e-30)
     cost_set = o_raw & t_raw & (o_k == t_k) & same_source
     depth_set = o_valid & t_valid & (o_k == t_k) & same_source
+    if depth_cond is not None:
+        allowed = DEPTH_RTOL + 3.0 * COST_TOL * depth_cond
+        depth_cond_viol = int((ddepth[depth_set] > allowed[depth_set]).sum())
+    else:
+        depth_cond_viol = -1
     raw_mismatch = (o_raw != t_raw)
     valid_mismatch = (o_valid != t_valid)
     stats = dict(
@@ -88,6 +110,7 @@ def compare_maps(orc: dict, test: dict, cost_volumes=None, index_flag_mask: int 
         max_dc2=float(dc2[cost_set & ~tie].max()) if (cost_set & ~tie).any() else 0.0,
         max_ddepth_rel=float(ddepth[depth_set].max()) if depth_set.any() else 0.0,
         frac_ddepth_over_tol=float((ddepth[depth_set] > DEPTH_RTOL).mean()) if depth_set.any() else 0.0,
+        depth_violations_conditioned=depth_cond_viol,
         fragile_frac=float(fragile_all.mean()),
         raw_valid_mismatch_nonfragile=int((raw_mismatch & ~(fragile)).sum()),
         valid_mismatch_nonfragile=int((valid_mismatch & ~fragile_all).sum()),

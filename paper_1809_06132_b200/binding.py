@@ -27,7 +27,7 @@ EXPORTS = (
     "fsw_ground_normal_in_ref", "fsw_planeset_create", "fsw_planeset_destroy", "fsw_planeset_size",
     "fsw_planeset_table", "fsw_context_create", "fsw_context_destroy", "fsw_compute_depth",
     "fsw_compute_depth_multires", "fsw_compute_depth_host", "fsw_compute_depth_multires_host",
-    "fsw_get_last_counters", "fsw_measure_fp32_peak",
+    "fsw_context_set_timing", "fsw_get_last_counters", "fsw_measure_fp32_peak",
 )
 
 
@@ -77,7 +77,7 @@ class CDepthOut(ctypes.Structure):
 
 class CCounters(ctypes.Structure):
     _fields_ = [("struct_size", ctypes.c_uint32), ("n_eval", ctypes.c_int64), ("n_raw_valid", ctypes.c_int64),
-                ("n_valid", ctypes.c_int64), ("n_launches", ctypes.c_int64)]
+                ("n_valid", ctypes.c_int64), ("n_launches", ctypes.c_int64), ("sweep_ms", ctypes.c_double)]
 
 
 _lib = None
@@ -115,6 +115,7 @@ def load_library():
     L.fsw_compute_depth_host.argtypes = single
     L.fsw_compute_depth_multires.argtypes = multi
     L.fsw_compute_depth_multires_host.argtypes = multi
+    L.fsw_context_set_timing.argtypes = [vp, i32]
     L.fsw_get_last_counters.argtypes = [vp, P(CCounters)]
     L.fsw_measure_fp32_peak.argtypes = [i32, vp, P(ctypes.c_double), P(ctypes.c_double)]
     for name in EXPORTS:
@@ -283,8 +284,18 @@ class Context:
             arr[i] = CImage(ptr, pitch, dt)
         return arr, keep
 
-    def _outputs(self, host, want):
+    def _outputs(self, host, want, out=None):
         torch = _torch()
+        if out is not None:  # caller-owned output tensors (e.g. pinned host buffers reused across calls)
+            c = CDepthOut()
+            c.struct_size = ctypes.sizeof(CDepthOut)
+            for name in ("depth", "best_cost", "second_cost", "plane_index", "valid_reason"):
+                t = out.get(name)
+                if t is not None:
+                    assert t.is_cuda != host and t.stride(1) == 1
+                    setattr(c, name, t.data_ptr())
+                    setattr(c, name + "_pitch", t.stride(0) * t.element_size())
+            return c, dict(out)
         W, H = self.rig.sizes[self.rig.ref_index]
         kw = dict(device="cpu", pin_memory=True) if host else dict(device="cuda:%d" % self.device)
         spec = dict(depth=torch.float32, best_cost=torch.float32, second_cost=torch.float32, plane_index=torch.int16,
@@ -315,14 +326,15 @@ class Context:
     ALL = ("best_cost", "second_cost", "plane_index", "valid_reason")
 
     # -- the calls of include/fsw.h ---------------------------------------------------------------------------------
-    def compute_depth(self, planes: PlaneSet, params, images, mask=None, want=ALL, host=False, debug_cost=False):
+    def compute_depth(self, planes: PlaneSet, params, images, mask=None, want=ALL, host=False, debug_cost=False,
+                      out=None):
         """fsw_compute_depth (device tensors) / fsw_compute_depth_host (host=True: numpy or CPU tensors).
         Returns a dict of tensors: depth (+ best_cost, second_cost, plane_index, valid_reason as requested)."""
         torch = _torch()
         L = load_library()
         arr, keep = self._images(images, host)
         mptr, mpitch, mkeep = self._mask(mask, host)
-        cout, out = self._outputs(host, want)
+        cout, out = self._outputs(host, want, out)
         dbg = None
         if debug_cost:
             assert not host
@@ -337,13 +349,13 @@ class Context:
         return out
 
     def compute_depth_multires(self, planes_low: PlaneSet, planes_crop: PlaneSet, params_low, params_crop, crop,
-                               images, mask=None, want=ALL, host=False):
+                               images, mask=None, want=ALL, host=False, out=None):
         """fsw_compute_depth_multires / _host: the two-scale strategy of PAPER.md:88-90."""
         torch = _torch()
         L = load_library()
         arr, keep = self._images(images, host)
         mptr, mpitch, mkeep = self._mask(mask, host)
-        cout, out = self._outputs(host, want)
+        cout, out = self._outputs(host, want, out)
         pl, pc = make_params(params_low), make_params(params_crop)
         stream = torch.cuda.current_stream(self.device).cuda_stream
         fn = L.fsw_compute_depth_multires_host if host else L.fsw_compute_depth_multires
@@ -356,7 +368,12 @@ class Context:
         c = CCounters()
         c.struct_size = ctypes.sizeof(CCounters)
         _check(load_library().fsw_get_last_counters(self.handle, ctypes.byref(c)))
-        return dict(n_eval=c.n_eval, n_raw_valid=c.n_raw_valid, n_valid=c.n_valid, n_launches=c.n_launches)
+        return dict(n_eval=c.n_eval, n_raw_valid=c.n_raw_valid, n_valid=c.n_valid, n_launches=c.n_launches,
+                    sweep_ms=c.sweep_ms)
+
+    def set_timing(self, on=True):
+        """fsw_context_set_timing: bracket the sweep kernels of later calls with CUDA events (last_counters()['sweep_ms'])."""
+        _check(load_library().fsw_context_set_timing(self.handle, 1 if on else 0))
 
 
 def measure_fp32_peak(device=0):

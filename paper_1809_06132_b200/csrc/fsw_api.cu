@@ -14,7 +14,7 @@
 
 /* per-window launchers, one object file each (fsw_sweep_inst.cu) */
 #define FSW_DECL_WIN(w)                                                               \
-    cudaError_t fsw_launch_sweep_w##w(const FswSweepArgs& args, cudaStream_t stream); \
+    cudaError_t fsw_launch_sweep_w##w(const FswSweepArgs& args, int variant, cudaStream_t stream); \
     cudaError_t fsw_prepare_sweep_w##w();
 FSW_DECL_WIN(3) FSW_DECL_WIN(5) FSW_DECL_WIN(7) FSW_DECL_WIN(9) FSW_DECL_WIN(11) FSW_DECL_WIN(13) FSW_DECL_WIN(15)
 #undef FSW_DECL_WIN
@@ -105,6 +105,9 @@ struct fsw_context {
     DevBuf st_img[FSW_MAX_CAMERAS], st_mask, st_depth, st_c1, st_c2, st_k, st_reason;
     cudaStream_t last_stream = nullptr;
     int64_t last_launches = 0;
+    bool timing = false, timed = false;
+    cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr}; /* [0,1] around the (crop) sweep, [2,3] around the low sweep */
+    int n_timed = 0;
     bool prepared[FSW_MAX_WINDOW + 1] = {false};
 };
 
@@ -284,15 +287,31 @@ cudaError_t prepare_window(fsw_context* ctx, int w) {
     return e;
 }
 
+/* picks the kernel variant the views allow (see fsw_sweep.cuh) */
+int pick_variant(const FswSweepArgs& a) {
+    bool ident = true, k1only = true, all_u8 = true, all_f32 = true;
+    for (int v = 0; v < a.n_views; ++v) {
+        ident = ident && a.views[v].ident_R;
+        k1only = k1only && a.views[v].cam.dist_mode != FSW_DIST_FULL;
+        k1only = k1only && (a.views[v].cam.cos_fov + a.views[v].cam.xi >= 1e-3f); /* lets the kernel drop the den test */
+        all_u8 = all_u8 && a.views[v].pix_mode == FSW_PIX_FOOT_U8;
+        all_f32 = all_f32 && a.views[v].pix_mode == FSW_PIX_F32;
+    }
+    if (ident && k1only && all_u8) return 1;
+    if (ident && k1only && all_f32) return 2;
+    return 0;
+}
+
 cudaError_t launch_window(const FswSweepArgs& a, int w, cudaStream_t s) {
+    const int var = pick_variant(a);
     switch (w) {
-        case 3: return fsw_launch_sweep_w3(a, s);
-        case 5: return fsw_launch_sweep_w5(a, s);
-        case 7: return fsw_launch_sweep_w7(a, s);
-        case 9: return fsw_launch_sweep_w9(a, s);
-        case 11: return fsw_launch_sweep_w11(a, s);
-        case 13: return fsw_launch_sweep_w13(a, s);
-        case 15: return fsw_launch_sweep_w15(a, s);
+        case 3: return fsw_launch_sweep_w3(a, var, s);
+        case 5: return fsw_launch_sweep_w5(a, var, s);
+        case 7: return fsw_launch_sweep_w7(a, var, s);
+        case 9: return fsw_launch_sweep_w9(a, var, s);
+        case 11: return fsw_launch_sweep_w11(a, var, s);
+        case 13: return fsw_launch_sweep_w13(a, var, s);
+        case 15: return fsw_launch_sweep_w15(a, var, s);
     }
     return cudaErrorInvalidValue;
 }
@@ -499,6 +518,8 @@ int32_t fsw_context_destroy(fsw_context* ctx) {
         ctx->foot[c].release(); ctx->half[c].release(); ctx->st_img[c].release();
     }
     ctx->lo_depth.release(); ctx->lo_c1.release(); ctx->lo_c2.release(); ctx->lo_k.release(); ctx->counters.release();
+    for (int i = 0; i < 4; ++i)
+        if (ctx->ev[i]) cudaEventDestroy(ctx->ev[i]);
     ctx->st_mask.release(); ctx->st_depth.release(); ctx->st_c1.release(); ctx->st_c2.release(); ctx->st_k.release(); ctx->st_reason.release();
     delete ctx;
     return FSW_OK;
@@ -529,7 +550,10 @@ int32_t fsw_compute_depth(fsw_context* ctx, const fsw_planeset* planes, const fs
     set_outputs(a, out, mask, mask_pitch);
     a.counters = (unsigned long long*)ctx->counters.p;
     a.count_pixels = 1;
+    ctx->n_timed = 0;
+    if (ctx->timing) FSW_CUDA(cudaEventRecord(ctx->ev[0], stream));
     FSW_CUDA(launch_window(a, params->window, stream));
+    if (ctx->timing) { FSW_CUDA(cudaEventRecord(ctx->ev[1], stream)); ctx->n_timed = 1; }
     ctx->last_launches++;
     return FSW_OK;
 }
@@ -597,7 +621,10 @@ int32_t fsw_compute_depth_multires(fsw_context* ctx, const fsw_planeset* planes_
     a.out_k = (int16_t*)ctx->lo_k.p; a.out_k_pitch = (int64_t)LW * 2;
     a.counters = (unsigned long long*)ctx->counters.p;
     a.count_pixels = 0;
+    ctx->n_timed = 0;
+    if (ctx->timing) FSW_CUDA(cudaEventRecord(ctx->ev[2], stream));
     FSW_CUDA(launch_window(a, params_low->window, stream));
+    if (ctx->timing) FSW_CUDA(cudaEventRecord(ctx->ev[3], stream));
     ctx->last_launches++;
 
     /* S10(d)-(e) + S9 + S11: full-resolution sweep inside the crop, merged with the upsampled maps in its epilogue */
@@ -614,7 +641,9 @@ int32_t fsw_compute_depth_multires(fsw_context* ctx, const fsw_planeset* planes_
     a.index_flag = FSW_INDEX_FROM_CROP;
     a.counters = (unsigned long long*)ctx->counters.p;
     a.count_pixels = 1;
+    if (ctx->timing) FSW_CUDA(cudaEventRecord(ctx->ev[0], stream));
     FSW_CUDA(launch_window(a, params_crop->window, stream));
+    if (ctx->timing) { FSW_CUDA(cudaEventRecord(ctx->ev[1], stream)); ctx->n_timed = 2; }
     ctx->last_launches++;
     return FSW_OK;
 }
@@ -682,6 +711,17 @@ int32_t fsw_compute_depth_multires_host(fsw_context* ctx, const fsw_planeset* pl
     return run_host(ctx, true, planes_low, planes_crop, params_low, params_crop, crop, images, mask, mask_pitch, out, cuda_stream);
 }
 
+int32_t fsw_context_set_timing(fsw_context* ctx, int32_t on) {
+    if (!ctx) return fail(FSW_E_INVALID_ARG, "fsw_context_set_timing: null context");
+    DeviceGuard g;
+    FSW_CUDA(g.enter(ctx->device));
+    if (on && !ctx->ev[0])
+        for (int i = 0; i < 4; ++i) FSW_CUDA(cudaEventCreate(&ctx->ev[i]));
+    ctx->timing = on != 0;
+    if (!on) ctx->n_timed = 0;
+    return FSW_OK;
+}
+
 int32_t fsw_get_last_counters(fsw_context* ctx, fsw_counters* out) {
     if (!ctx || !out) return fail(FSW_E_INVALID_ARG, "fsw_get_last_counters: null argument");
     if (out->struct_size != sizeof(fsw_counters)) return fail(FSW_E_INVALID_ARG, "fsw_get_last_counters: struct_size %u != %zu", out->struct_size, sizeof(fsw_counters));
@@ -694,6 +734,13 @@ int32_t fsw_get_last_counters(fsw_context* ctx, fsw_counters* out) {
     out->n_raw_valid = (int64_t)h[1];
     out->n_valid = (int64_t)h[2];
     out->n_launches = ctx->last_launches;
+    out->sweep_ms = -1.0;
+    if (ctx->n_timed > 0) {
+        float t = 0.f, t2 = 0.f;
+        FSW_CUDA(cudaEventElapsedTime(&t, ctx->ev[0], ctx->ev[1]));
+        if (ctx->n_timed > 1) FSW_CUDA(cudaEventElapsedTime(&t2, ctx->ev[2], ctx->ev[3]));
+        out->sweep_ms = (double)t + (double)t2;
+    }
     return FSW_OK;
 }
 

@@ -51,7 +51,7 @@ struct Cfg {
     static constexpr int SB = (SB1 >= (NRUN - 1) * RUN + NV4 * 4) ? SB1 : SB1 + 8;
     static constexpr int PLANE = EH * SB;          /* floats in one sample plane */
     static constexpr int HPLANE = EH * HS;         /* floats in one row-sum plane */
-    static constexpr size_t SMEM = sizeof(float4) * NE + sizeof(float) * (2 * PLANE + 4 * HPLANE);
+    static constexpr size_t SMEM = sizeof(float4) * PLANE + sizeof(float) * (2 * PLANE + 4 * HPLANE);
 };
 
 __device__ __forceinline__ float rsqrt_approx(float x) {
@@ -122,72 +122,111 @@ __device__ inline bool back_project(const FswDevCam& c, float u, float v, float&
     return rz >= c.cos_fov; /* theta <= fov/2 */
 }
 
-/* S2-S4 for one halo pixel: returns the bilinear sample of the view at the plane-induced position, or NaN if the
- * pixel / plane / view combination is invalid ("NONE" of SURVEY 8(b)). */
-__device__ __forceinline__ float warp_sample(const float4 ray, const FswDevView& vw, float nx, float ny, float nz,
-                                             float inv_d, float inv_range_max, float centre) {
+/* Per-view constants of the sample phase, copied out of the kernel arguments once per (plane, view). */
+struct ViewK {
+    float T0, T1, T2;
+    float R[9];
+    float fx, fy, cx, cy, xi, cos_fov, k1, k2, p1, p2;
+    unsigned W1, H1; /* W-1, H-1 */
+    const void* img;
+    int pitch, pix;
+};
+
+__device__ __forceinline__ ViewK load_view(const FswDevView& vw) {
+    ViewK k;
+    k.T0 = vw.T[0]; k.T1 = vw.T[1]; k.T2 = vw.T[2];
+#pragma unroll
+    for (int i = 0; i < 9; ++i) k.R[i] = vw.R[i];
+    k.fx = vw.cam.fx; k.fy = vw.cam.fy; k.cx = vw.cam.cx; k.cy = vw.cam.cy; k.xi = vw.cam.xi;
+    k.cos_fov = vw.cam.cos_fov; k.k1 = vw.cam.k1; k.k2 = vw.cam.k2; k.p1 = vw.cam.p1; k.p2 = vw.cam.p2;
+    k.W1 = (unsigned)(vw.cam.W - 1); k.H1 = (unsigned)(vw.cam.H - 1);
+    k.img = vw.img; k.pitch = (int)vw.pitch_elems; k.pix = vw.pix_mode;
+    return k;
+}
+
+/* S2-S4 for one halo pixel: returns the bilinear sample of the view at the plane-induced position minus `centre`,
+ * or NaN if the pixel / plane / view combination is invalid ("NONE" of SURVEY 8(b)).
+ * IDENT: the view's relative rotation is the identity.  FULLDIST: k2 / p1 / p2 may be non-zero.
+ * PIX: FSW_PIX_FOOT_U8, FSW_PIX_F32, or -1 = decided per view at run time.
+ * cbias = 2^23 + rint(centre): 8-bit samples are widened by OR-ing them into the mantissa of 2^23, so subtracting
+ * cbias both removes that bias and centres the sample, exactly. */
+template <bool IDENT, bool FULLDIST, int PIX, bool CHECKDEN>
+__device__ __forceinline__ float warp_sample(const float4 ray, const ViewK& k, float nx, float ny, float nz,
+                                             float inv_d, float inv_range_max, float centre, float cbias) {
     /* S2: incidence and inverse range; X' ~ R r + (q/d) T */
     float q = fmaf(nx, ray.x, fmaf(ny, ray.y, nz * ray.z));
     float s = q * inv_d;
-    bool ok = (ray.w != 0.f) & (q > FSW_EPS_Q) & (s >= inv_range_max);
+    bool ok = (q > FSW_EPS_Q) & (s >= inv_range_max); /* an invalid reference ray is stored as 0: q = 0 */
     float X, Y, Z;
-    if (vw.ident_R) {
-        X = fmaf(s, vw.T[0], ray.x);
-        Y = fmaf(s, vw.T[1], ray.y);
-        Z = fmaf(s, vw.T[2], ray.z);
+    if (IDENT) {
+        X = fmaf(s, k.T0, ray.x);
+        Y = fmaf(s, k.T1, ray.y);
+        Z = fmaf(s, k.T2, ray.z);
     } else {
-        X = fmaf(vw.R[0], ray.x, fmaf(vw.R[1], ray.y, fmaf(vw.R[2], ray.z, s * vw.T[0])));
-        Y = fmaf(vw.R[3], ray.x, fmaf(vw.R[4], ray.y, fmaf(vw.R[5], ray.z, s * vw.T[1])));
-        Z = fmaf(vw.R[6], ray.x, fmaf(vw.R[7], ray.y, fmaf(vw.R[8], ray.z, s * vw.T[2])));
+        X = fmaf(k.R[0], ray.x, fmaf(k.R[1], ray.y, fmaf(k.R[2], ray.z, s * k.T0)));
+        Y = fmaf(k.R[3], ray.x, fmaf(k.R[4], ray.y, fmaf(k.R[5], ray.z, s * k.T1)));
+        Z = fmaf(k.R[6], ray.x, fmaf(k.R[7], ray.y, fmaf(k.R[8], ray.z, s * k.T2)));
     }
-    /* S3: unified projection */
-    const FswDevCam& c = vw.cam;
+    /* S3: unified projection; one Newton step on each approximate reciprocal */
     float rho2 = fmaf(X, X, fmaf(Y, Y, Z * Z));
+#ifdef FSW_REFINE_RECIPROCALS
+    float y0 = rsqrt_approx(rho2);
+    float t0 = rho2 * y0;
+    float rho = fmaf(0.5f * t0, fmaf(-t0, y0, 1.f), t0);
+#else
     float rho = rho2 * rsqrt_approx(rho2);
-    float den = fmaf(c.xi, rho, Z);
-    ok &= (den > FSW_EPS_DEN * rho) & (Z >= c.cos_fov * rho);
+#endif
+    float den = fmaf(k.xi, rho, Z);
+    ok &= (Z >= k.cos_fov * rho); /* also false for NaN (rho2 == 0) */
+    /* with cos(fov/2) + xi >= 1e-3 (checked on the host for the fast variants) the FOV test implies den > eps rho */
+    if (CHECKDEN) ok &= (den > FSW_EPS_DEN * rho);
+#ifdef FSW_REFINE_RECIPROCALS
+    float i0 = rcp_approx(den);
+    float iden = fmaf(i0, fmaf(-den, i0, 1.f), i0);
+#else
     float iden = rcp_approx(den);
+#endif
     float mx = X * iden, my = Y * iden;
-    float xd = mx, yd = my;
-    if (c.dist_mode != FSW_DIST_NONE) {
-        float r2 = fmaf(mx, mx, my * my);
-        if (c.dist_mode == FSW_DIST_K1) {
-            float rad = fmaf(c.k1, r2, 1.f);
-            xd = mx * rad;
-            yd = my * rad;
-        } else {
-            float rad = fmaf(r2, fmaf(c.k2, r2, c.k1), 1.f);
-            xd = fmaf(mx, rad, fmaf(2.f * c.p1 * mx, my, c.p2 * fmaf(2.f * mx, mx, r2)));
-            yd = fmaf(my, rad, fmaf(c.p1, fmaf(2.f * my, my, r2), 2.f * c.p2 * mx * my));
-        }
+    float r2 = fmaf(mx, mx, my * my);
+    float xd, yd;
+    if (!FULLDIST) {
+        float rad = fmaf(k.k1, r2, 1.f);
+        xd = mx * rad;
+        yd = my * rad;
+    } else {
+        float rad = fmaf(r2, fmaf(k.k2, r2, k.k1), 1.f);
+        xd = fmaf(mx, rad, fmaf(2.f * k.p1 * mx, my, k.p2 * fmaf(2.f * mx, mx, r2)));
+        yd = fmaf(my, rad, fmaf(k.p1, fmaf(2.f * my, my, r2), 2.f * k.p2 * mx * my));
     }
-    float u = fmaf(c.fx, xd, c.cx);
-    float v = fmaf(c.fy, yd, c.cy);
-    /* bilinear footprint inside the view image: 0 <= u < W-1, 0 <= v < H-1 */
-    ok &= (u >= 0.f) & (u < (float)(c.W - 1)) & (v >= 0.f) & (v < (float)(c.H - 1));
+    float u = fmaf(k.fx, xd, k.cx);
+    float v = fmaf(k.fy, yd, k.cy);
+    /* bilinear footprint inside the view image: 0 <= u < W-1, 0 <= v < H-1  <=>  0 <= floor(u) < W-1, ... */
+    int ix = __float2int_rd(u), iy = __float2int_rd(v);
+    ok &= ((unsigned)ix < k.W1) & ((unsigned)iy < k.H1);
     float b = CUDART_NAN_F;
     if (ok) {
-        /* S4: four point fetches, FP32 lerp (hardware texture filtering has 8-bit weights: too coarse) */
-        float fu = floorf(u), fv = floorf(v);
-        int ix = (int)fu, iy = (int)fv;
-        float au = u - fu, av = v - fv;
-        float i00, i10, i01, i11;
-        if (vw.pix_mode == FSW_PIX_FOOT_U8) {
-            uint32_t w = __ldg(reinterpret_cast<const uint32_t*>(vw.img) + (int64_t)iy * vw.pitch_elems + ix);
-            i00 = (float)(w & 0xffu);
-            i10 = (float)((w >> 8) & 0xffu);
-            i01 = (float)((w >> 16) & 0xffu);
-            i11 = (float)(w >> 24);
+        /* S4: point fetches + FP32 lerp (hardware texture filtering has 8-bit weights: too coarse for 1e-4) */
+        float au = u - (__int_as_float(ix + 0x4B400000) - 12582912.f); /* u - floor(u) without a second conversion */
+        float av = v - (__int_as_float(iy + 0x4B400000) - 12582912.f);
+        int idx = iy * k.pitch + ix;
+        float i00, d0, i01, d1;
+        if (PIX == FSW_PIX_FOOT_U8 || (PIX < 0 && k.pix == FSW_PIX_FOOT_U8)) {
+            uint32_t w = __ldg(reinterpret_cast<const uint32_t*>(k.img) + idx);
+            float f00 = __uint_as_float(__byte_perm(w, 0x4B000000u, 0x7540));
+            float f10 = __uint_as_float(__byte_perm(w, 0x4B000000u, 0x7541));
+            float f01 = __uint_as_float(__byte_perm(w, 0x4B000000u, 0x7542));
+            float f11 = __uint_as_float(__byte_perm(w, 0x4B000000u, 0x7543));
+            i00 = f00 - cbias; d0 = f10 - f00;
+            i01 = f01 - cbias; d1 = f11 - f01;
         } else {
-            const float* p = reinterpret_cast<const float*>(vw.img) + (int64_t)iy * vw.pitch_elems + ix;
-            i00 = __ldg(p);
-            i10 = __ldg(p + 1);
-            i01 = __ldg(p + vw.pitch_elems);
-            i11 = __ldg(p + vw.pitch_elems + 1);
+            const float* p = reinterpret_cast<const float*>(k.img) + idx;
+            float f00 = __ldg(p), f10 = __ldg(p + 1), f01 = __ldg(p + k.pitch), f11 = __ldg(p + k.pitch + 1);
+            i00 = f00 - centre; d0 = f10 - f00;
+            i01 = f01 - centre; d1 = f11 - f01;
         }
-        float top = fmaf(au, i10 - i00, i00);
-        float bot = fmaf(au, i11 - i01, i01);
-        b = fmaf(av, bot - top, top) - centre;
+        float top = fmaf(au, d0, i00);
+        float bot = fmaf(au, d1, i01);
+        b = fmaf(av, bot - top, top);
     }
     return b;
 }
@@ -270,14 +309,17 @@ __device__ __forceinline__ void vpass(const float* __restrict__ h, int x, int r0
     }
 }
 
-template <int WIN>
+/* warp-uniform value that the compiler can also prove uniform (lets it keep loop state in uniform registers) */
+__device__ __forceinline__ int uniform_int(int x) { return __shfl_sync(0xffffffffu, x, 0); }
+
+template <int WIN, bool IDENT, bool FULLDIST, int PIX, bool CHECKDEN>
 __global__ void __launch_bounds__(NT, 2) sweep_kernel(const __grid_constant__ FswSweepArgs args) {
     using C = Cfg<WIN>;
     constexpr int HW = C::HW;
     constexpr float NWIN = (float)(WIN * WIN);
     extern __shared__ __align__(16) unsigned char smem_raw[];
     float4* rays = reinterpret_cast<float4*>(smem_raw);
-    float* a_s = reinterpret_cast<float*>(rays + C::NE);
+    float* a_s = reinterpret_cast<float*>(rays + C::PLANE);
     float* b_s = a_s + C::PLANE;
     float* hs = b_s + C::PLANE;
     __shared__ float red_sum[NT / 32];
@@ -311,24 +353,28 @@ __global__ void __launch_bounds__(NT, 2) sweep_kernel(const __grid_constant__ Fs
         /* ---- S1: rays and reference intensities of the tile + halo ------------------------------------ */
         float lsum = 0.f;
         int lcnt = 0;
-        for (int e = tid; e < C::NE; e += NT) {
-            int row = e / C::EW, col = e - row * C::EW;
+        int my_n = 0; /* halo pixels (not pad entries) this thread samples per plane and view */
+        for (int p = tid; p < C::PLANE; p += NT) {
+            int row = p / C::SB, col = p - row * C::SB;
             int px = x0t - HW + col, py = y0t - HW + row;
-            float4 ry = make_float4(0.f, 0.f, 0.f, 0.f);
+            float4 ry = make_float4(0.f, 0.f, 0.f, 0.f); /* invalid rays (and pad entries) are zero vectors */
             float a = 0.f;
-            if (px >= 0 && px < W && py >= 0 && py < H) {
-                float rx, ryy, rz;
-                if (back_project(args.ref, (float)px, (float)py, rx, ryy, rz)) ry = make_float4(rx, ryy, rz, 1.f);
-                if (args.ref_dtype == FSW_U8)
-                    a = (float)__ldg(reinterpret_cast<const uint8_t*>(args.ref_img) + (int64_t)py * args.ref_pitch_bytes + px);
-                else
-                    a = __ldg(reinterpret_cast<const float*>(reinterpret_cast<const char*>(args.ref_img) + (int64_t)py * args.ref_pitch_bytes) + px);
-                lsum += a;
-                lcnt += 1;
+            if (col < C::EW) {
+                my_n += 1;
+                if (px >= 0 && px < W && py >= 0 && py < H) {
+                    float rx, ryy, rz;
+                    bool ok = back_project(args.ref, (float)px, (float)py, rx, ryy, rz);
+                    if (ok) ry = make_float4(rx, ryy, rz, 1.f);
+                    if (args.ref_dtype == FSW_U8)
+                        a = (float)__ldg(reinterpret_cast<const uint8_t*>(args.ref_img) + (int64_t)py * args.ref_pitch_bytes + px);
+                    else
+                        a = __ldg(reinterpret_cast<const float*>(reinterpret_cast<const char*>(args.ref_img) + (int64_t)py * args.ref_pitch_bytes) + px);
+                    if (ok) { lsum += a; lcnt += 1; } /* pixels outside the FOV never enter a valid window */
+                }
             }
-            rays[e] = ry;
-            a_s[row * C::SB + col] = a;
-            b_s[row * C::SB + col] = ry.w;
+            rays[p] = ry;
+            a_s[p] = a;
+            b_s[p] = ry.w;
         }
         /* centring constant of the tile: mean reference intensity (rounded to an integer for 8-bit images so
          * that a - centre stays exact) */
@@ -345,10 +391,8 @@ __global__ void __launch_bounds__(NT, 2) sweep_kernel(const __grid_constant__ Fs
         for (int i = 0; i < NT / 32; ++i) { tsum += red_sum[i]; tcnt += red_cnt[i]; }
         float centre = tcnt > 0 ? tsum / (float)tcnt : 0.f;
         if (args.ref_dtype == FSW_U8) centre = rintf(centre);
-        for (int e = tid; e < C::NE; e += NT) {
-            int row = e / C::EW, col = e - row * C::EW;
-            a_s[row * C::SB + col] -= centre;
-        }
+        const float cbias = 8388608.f + rintf(centre);
+        for (int p = tid; p < C::PLANE; p += NT) a_s[p] -= centre;
         __syncthreads();
         /* window sums of the reference side, once per pixel: A1 = sum a', A2 = N sum a'^2 - (sum a')^2 */
         if (tid < C::EH * NRUN) hpass<WIN, 0>(a_s, b_s, hs, tid);
@@ -368,7 +412,7 @@ __global__ void __launch_bounds__(NT, 2) sweep_kernel(const __grid_constant__ Fs
                 A2[i] = fmaf(NWIN, saa[i], -sa[i] * sa[i]);
             }
         }
-        tile_active = __syncthreads_or(active_mask != 0);
+        tile_active = uniform_int(__syncthreads_or(active_mask != 0)) != 0;
 
         if (tile_active) {
             const float inv_views = 1.f / (float)args.n_views;
@@ -380,11 +424,11 @@ __global__ void __launch_bounds__(NT, 2) sweep_kernel(const __grid_constant__ Fs
                 for (int i = 0; i < RPT; ++i) { m1[i] = m0[i]; cprev[i] = CUDART_INF_F; knext[i] = -1; }
                 /* does any halo ray face this family's planes? */
                 bool faces = false;
-                for (int e = tid; e < C::NE; e += NT) {
-                    float4 ry = rays[e];
+                for (int p = tid; p < C::PLANE; p += NT) {
+                    float4 ry = rays[p];
                     faces |= (ry.w != 0.f) && (fmaf(nx, ry.x, fmaf(ny, ry.y, nz * ry.z)) > FSW_EPS_Q);
                 }
-                const bool fam_active = __syncthreads_or(faces);
+                const bool fam_active = uniform_int(__syncthreads_or(faces)) != 0;
                 for (int j = 0; j < F.count; ++j) {
                     const int k = F.first + j;
                     const float inv_d = args.inv_d[k];
@@ -394,21 +438,20 @@ __global__ void __launch_bounds__(NT, 2) sweep_kernel(const __grid_constant__ Fs
                     for (int i = 0; i < RPT; ++i) { acc[i] = 0.f; cnt[i] = 0; }
                     if (fam_active) {
                         for (int v = 0; v < args.n_views; ++v) {
-                            const FswDevView& vw = args.views[v];
+                            const ViewK vk = load_view(args.views[v]);
                             /* ---- S2-S4: sample the plane-warped view at every halo pixel -------------------- */
-                            bool all_ok = true, any_ok = false;
-                            for (int e = tid; e < C::NE; e += NT) {
-                                int row = e / C::EW, col = e - row * C::EW;
-                                float b = warp_sample(rays[e], vw, nx, ny, nz, inv_d, args.inv_range_max, centre);
-                                bool ok = (b == b);
-                                all_ok &= ok;
-                                any_ok |= ok;
-                                b_s[row * C::SB + col] = b;
+                            int nvalid = 0;
+#pragma unroll 2
+                            for (int p = tid; p < C::PLANE; p += NT) {
+                                float b = warp_sample<IDENT, FULLDIST, PIX, CHECKDEN>(rays[p], vk, nx, ny, nz, inv_d,
+                                                                                      args.inv_range_max, centre, cbias);
+                                nvalid += (b == b) ? 1 : 0;
+                                b_s[p] = b;
                             }
-                            const int n_all = __syncthreads_count(all_ok);
+                            const int n_all = uniform_int(__syncthreads_count(nvalid == my_n));
                             const bool mixed = n_all != NT;
                             if (mixed) {
-                                if (!__syncthreads_or(any_ok)) continue; /* this view sees nothing of the tile */
+                                if (!uniform_int(__syncthreads_or(nvalid > 0))) continue; /* this view sees nothing of the tile */
                             }
                             /* ---- S5: separable box sums and ZNCC ------------------------------------------- */
                             if (tid < C::EH * NRUN) {
@@ -490,7 +533,7 @@ __global__ void __launch_bounds__(NT, 2) sweep_kernel(const __grid_constant__ Fs
             }
             float s = fmaf((float)(k1[i] - F.first) + dl, F.ds, F.s0);
             float d = F.spacing == FSW_INVERSE ? 1.f / s : s;
-            float4 ry = rays[(wy * RPT + i + HW) * C::EW + lane + HW];
+            float4 ry = rays[(wy * RPT + i + HW) * C::SB + lane + HW];
             float q = fmaf(F.n[0], ry.x, fmaf(F.n[1], ry.y, F.n[2] * ry.z));
             float range = d / q;
             depth = args.depth_kind == FSW_DEPTH_Z ? range * ry.z : range;
@@ -543,16 +586,25 @@ __global__ void __launch_bounds__(NT, 2) sweep_kernel(const __grid_constant__ Fs
     }
 }
 
+/* Kernel variants: 0 = generic (any rotation, full distortion polynomial, pixel type decided per view),
+ * 1 = identity rotations, k1-only (or no) distortion, cos(fov/2) + xi >= 1e-3, footprint-packed 8-bit views,
+ * 2 = the same with float32 views. */
 template <int WIN>
-cudaError_t launch_sweep_win(const FswSweepArgs& args, cudaStream_t stream) {
+cudaError_t launch_sweep_win(const FswSweepArgs& args, int variant, cudaStream_t stream) {
     dim3 grid((args.ref.W + TX - 1) / TX, (args.ref.H + TY - 1) / TY);
-    sweep_kernel<WIN><<<grid, NT, Cfg<WIN>::SMEM, stream>>>(args);
+    if (variant == 1) sweep_kernel<WIN, true, false, FSW_PIX_FOOT_U8, false><<<grid, NT, Cfg<WIN>::SMEM, stream>>>(args);
+    else if (variant == 2) sweep_kernel<WIN, true, false, FSW_PIX_F32, false><<<grid, NT, Cfg<WIN>::SMEM, stream>>>(args);
+    else sweep_kernel<WIN, false, true, -1, true><<<grid, NT, Cfg<WIN>::SMEM, stream>>>(args);
     return cudaGetLastError();
 }
 
 template <int WIN>
 cudaError_t prepare_sweep_win() {
-    return cudaFuncSetAttribute(sweep_kernel<WIN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg<WIN>::SMEM);
+    cudaError_t e = cudaFuncSetAttribute(sweep_kernel<WIN, true, false, FSW_PIX_FOOT_U8, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg<WIN>::SMEM);
+    if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(sweep_kernel<WIN, true, false, FSW_PIX_F32, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg<WIN>::SMEM);
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(sweep_kernel<WIN, false, true, -1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg<WIN>::SMEM);
 }
 
 }  // namespace fsw

@@ -11,7 +11,7 @@
 #define FSW_CAT2(a, b) a##b
 #define FSW_CAT(a, b) FSW_CAT2(a, b)
 
-cudaError_t FSW_CAT(fsw_launch_sweep_w, FSW_WIN)(const FswSweepArgs& args, cudaStream_t stream) {
-    return fsw::launch_sweep_win<FSW_WIN>(args, stream);
+cudaError_t FSW_CAT(fsw_launch_sweep_w, FSW_WIN)(const FswSweepArgs& args, int variant, cudaStream_t stream) {
+    return fsw::launch_sweep_win<FSW_WIN>(args, variant, stream);
 }
 cudaError_t FSW_CAT(fsw_prepare_sweep_w, FSW_WIN)() { return fsw::prepare_sweep_win<FSW_WIN>(); }

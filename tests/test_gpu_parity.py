@@ -1,0 +1,202 @@
+"""-m gpu: the CUDA path, called through the C ABI, against the oracle on the same seeded inputs.
+
+Gates (BASELINE.json north_star; derivations in DESIGN.md "Tolerances"):
+  index   >= 99.9 % of oracle-valid pixels, a differing index only as a tie in the oracle's own cost vector (2e-4)
+  cost    |c1 - c1_oracle| <= 1e-4 wherever the indices agree
+  depth   within 1e-3 relative on >= 99.9 % of the pixels whose indices agree, and on ALL of them within
+          1e-3 + 3e-4 * (|ds|/s) / pden  (the parabola's conditioning at the 1e-4 cost tolerance)
+  valid   bit-exact on pixels the oracle does not mark fragile
+  N_eval  the kernel's counter of finite (pixel, plane, view) costs equals the oracle's within 0.1 %
+"""
+import numpy as np
+import pytest
+
+import oracle
+import synth
+from parity_helpers import assert_gates, gpu_objects, run_multires, run_single
+
+pytestmark = pytest.mark.gpu
+
+
+def _small_rig(W=70, H=45, n_views=1, xi=0.9, rot=False, dist=None, dtype="u8", seed=7, fov=200.0):
+    """A small seeded rig + plane scene whose sizes are not multiples of the 32x32 tile (ragged tails)."""
+    kw = dict(width=W, height=H, fx=0.45 * W, fy=0.45 * W, cx=W / 2.0 - 0.3, cy=H / 2.0 + 0.2, xi=xi, fov_max_deg=fov)
+    if dist:
+        kw.update(dist)
+    centres = [(0.3, 0, 0), (-0.25, 0.05, 0), (0.0, -0.3, 0.02), (0.2, 0.2, 0)][:n_views]
+    yaws = [8.0, -6.0, 3.0, -2.0] if rot else [0.0] * 4
+    cams = [synth.camera(**kw)] + [synth.camera(centre=c, yaw_deg=yaws[i], **kw) for i, c in enumerate(centres)]
+    cfg = dict(name="small", dtype=dtype, ref_index=0, cams=cams,
+               families=[synth.family((0, 0, 1), 24, 0.8, 30.0, "inverse")],
+               params=synth.params(5, synth.VAR_FLOOR_U8 if dtype == "u8" else synth.VAR_FLOOR_F32, 60.0),
+               scene=synth.scene_plane(3.0, (0.5, 2.0), seed=seed))
+    return cfg
+
+
+# ---- the five BASELINE.json configs ---------------------------------------------------------------------------------
+@pytest.mark.parametrize("idx", [1, 2, 3])
+def test_config_single_resolution(idx):
+    cfg = synth.make_config(idx)
+    images = synth.render_frame(cfg, 0)
+    _, _, stats, counters = run_single(cfg, images)
+    assert_gates(stats)
+    assert counters["n_launches"] >= 1
+
+
+@pytest.mark.parametrize("idx", [1, 2])
+def test_config_with_filters(idx):
+    """C1 / C2 name no filters; SURVEY 8(d) asks for both the raw-valid set and alpha = 0.3/0.3, beta = 1.2."""
+    cfg = synth.make_config(idx)
+    images = synth.render_frame(cfg, 0)
+    p = dict(cfg["params"], alpha_upper=0.3, alpha_lower=0.3, beta=1.2, filters=3, horizon_row=cfg["cams"][0]["height"] // 2)
+    ref, test, stats, _ = run_single(cfg, images, params=p)
+    assert_gates(stats)
+    assert 0 < stats["n_oracle_valid"] < stats["n_oracle_raw_valid"]
+
+
+def test_config4_multires_merge_and_mask():
+    cfg = synth.make_config(4)
+    images = synth.render_frame(cfg, 0)
+    mask = synth.make_mask(1280, 1024, cfg["mask_seed"])
+    ref, test, stats, counters = run_multires(cfg, images, mask)
+    assert_gates(stats)
+    # outside the crop every value is the nearest-neighbour upsampled half-resolution one (no crop flag)
+    x0, y0, w, h = cfg["crop"]
+    outside = np.ones(mask.shape, bool)
+    outside[y0:y0 + h, x0:x0 + w] = False
+    k = test["plane_index"].astype(np.int32)
+    assert not ((k[outside] >= 0) & ((k[outside] >> 14) & 1).astype(bool)).any()
+    assert (test["depth"][mask != 0] == 0).all() and (test["valid_reason"][mask != 0] != 0).all()
+    assert counters["n_launches"] == 4  # downsample, low sweep, footprint pack, crop sweep
+
+
+@pytest.mark.parametrize("frame", [0, 31])
+def test_config5_stream_frames(frame):
+    cfg = synth.make_config(5)
+    images = synth.render_frame(cfg, frame)
+    mask = synth.make_mask(1280, 1024, cfg["mask_seed"] + frame)
+    _, test, stats, _ = run_single(cfg, images, mask)
+    assert_gates(stats)
+    assert (test["depth"][mask != 0] == 0).all()
+
+
+# ---- cost volume, element by element --------------------------------------------------------------------------------
+def test_debug_cost_volume_matches_oracle():
+    cfg = synth.make_config(2)
+    images = synth.render_frame(cfg, 0)
+    ref, test, stats, _ = run_single(cfg, images, debug_cost=True)
+    vol, ovol = test["cost_volume"].astype(np.float64), ref["cost"]
+    fin_o, fin_t = np.isfinite(ovol), np.isfinite(vol)
+    frag = ref["fragile_geom"] != 0
+    assert not ((fin_o != fin_t) & ~frag[None]).any()
+    both = fin_o & fin_t
+    assert np.abs(vol[both] - ovol[both]).max() <= 1e-4
+    assert_gates(stats)
+
+
+# ---- edge cases ---------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("window", [3, 5, 7, 9, 11, 13, 15])
+def test_every_window_size_ragged_image(window):
+    cfg = _small_rig(W=70, H=45)
+    cfg["params"] = dict(cfg["params"], window=window)
+    images = synth.render_frame(cfg, 0)
+    _, _, stats, _ = run_single(cfg, images)
+    assert_gates(stats, depth_frac_over_tol=0.001 if window >= 5 else 0.01)
+    assert stats["n_oracle_valid"] > 0
+
+
+@pytest.mark.parametrize("n_views,rot,dist,dtype", [
+    (1, False, None, "f32"),
+    (3, True, None, "u8"),
+    (2, True, dict(k1=-0.03, k2=0.004, p1=0.0008, p2=-0.0006), "u8"),
+    (4, True, dict(k1=-0.04), "f32"),
+])
+def test_views_rotation_distortion_dtype(n_views, rot, dist, dtype):
+    cfg = _small_rig(W=96, H=64, n_views=n_views, rot=rot, dist=dist, dtype=dtype, fov=170.0)
+    images = synth.render_frame(cfg, 0)
+    _, _, stats, _ = run_single(cfg, images)
+    assert_gates(stats)
+    assert stats["n_oracle_valid"] > 500
+
+
+def test_two_families_linear_ground_roi_z_depth_no_subpixel():
+    cfg = synth.make_config(2)
+    images = synth.render_frame(cfg, 0)
+    fams = [synth.family((0, 0, 1), 20, 1.0, 40.0, "inverse"), synth.family((0, 1, 0), 9, 1.2, 2.0, "linear"),
+            synth.family((0, 0, 1), 1, 2.5, 2.5, "linear")]
+    for sub, kind in ((1, 1), (0, 0)):
+        p = dict(cfg["params"], roi=(37, 21, 201, 150), depth_kind=kind, subpixel=sub, filters=3, alpha_upper=0.2,
+                 alpha_lower=0.35, beta=1.1, horizon_row=100)
+        ref, test, stats, _ = run_single(cfg, images, params=p, families=fams)
+        assert_gates(stats)
+        outside = np.ones(ref["depth"].shape, bool)
+        outside[21:21 + 150, 37:37 + 201] = False
+        assert (test["depth"][outside] == 0).all() and (test["plane_index"][outside] == -1).all()
+        assert (ref["kbest"] >= 20).any()  # the ground family wins somewhere
+
+
+def test_degenerate_inputs():
+    import torch
+    import paper_1809_06132_b200 as fsw
+    cfg = _small_rig(W=64, H=48)
+    fsw_mod, rig, ctx = gpu_objects(cfg)
+    images = synth.render_frame(cfg, 0)
+    # (a) everything masked -> all invalid, reasons say why
+    mask = np.ones((48, 64), np.uint8)
+    ref, test, stats, _ = run_single(cfg, images, mask, ctx=ctx)
+    assert (test["depth"] == 0).all() and stats["valid_mismatch_total"] == 0
+    assert set(np.unique(test["valid_reason"])) <= {fsw.REASON_NO_PLANE, fsw.REASON_MASKED}
+    # (b) constant images: cost = 0.5 on every plane, lowest index wins, the cost filter rejects everything
+    flat = [np.full((48, 64), 90, np.uint8)] * 2
+    p = dict(cfg["params"], filters=1, alpha_upper=0.3, alpha_lower=0.3)
+    ref, test, stats, _ = run_single(cfg, flat, params=p, ctx=ctx)
+    assert (test["depth"] == 0).all() and stats["valid_mismatch_total"] == 0
+    k = test["plane_index"]
+    assert np.array_equal(k[k >= 0], ref["kbest"][ref["kbest"] >= 0])
+    assert np.abs(test["best_cost"][k >= 0] - 0.5).max() < 1e-6
+    # (c) ROI entirely outside the field of view / clipped away -> no plane anywhere, nothing evaluated
+    p = dict(cfg["params"], roi=(0, 0, 3, 3))
+    ref, test, stats, counters = run_single(cfg, images, params=p, ctx=ctx)
+    assert (test["plane_index"] == -1).all() and counters["n_eval"] == 0 and ref["n_eval"] == 0
+    # (d) the largest plane set the ABI accepts
+    fams = [synth.family((0, 0, 1), 1024, 0.8, 30.0, "inverse")]
+    ref, test, stats, _ = run_single(cfg, images, families=fams, ctx=ctx)
+    assert_gates(stats, depth_frac_over_tol=0.05)  # 1024 planes over 64x48 pixels: every cost curve is flat
+    # (e) bad arguments are errors, not crashes
+    planes = fsw.PlaneSet(cfg["families"])
+    dev = [torch.from_numpy(im).cuda() for im in images]
+    for bad in (dict(window=4), dict(window=17), dict(range_max=0.0), dict(filters=8)):
+        with pytest.raises(fsw.FswError) as ei:
+            ctx.compute_depth(planes, dict(cfg["params"], **bad), dev)
+        assert ei.value.code == fsw.binding.E_INVALID_ARG
+
+
+def test_host_call_equals_device_call_and_is_deterministic():
+    cfg = synth.make_config(2)
+    images = synth.render_frame(cfg, 0)
+    _, _, ctx = gpu_objects(cfg)
+    p = dict(cfg["params"], filters=3, alpha_upper=0.3, alpha_lower=0.3, beta=1.2, horizon_row=128)
+    _, a, _, _ = run_single(cfg, images, params=p, ctx=ctx)
+    _, b, _, _ = run_single(cfg, images, params=p, ctx=ctx, host=True)
+    _, c, _, _ = run_single(cfg, images, params=p, ctx=ctx)
+    for key in ("depth", "best_cost", "second_cost", "plane_index", "valid_reason"):
+        assert np.array_equal(a[key], b[key], equal_nan=True), key
+        assert np.array_equal(a[key], c[key], equal_nan=True), key
+
+
+def test_multires_host_call_small():
+    """S10 on a small rig: host-buffer call, crop not aligned to the tile grid, odd crop origin."""
+    cfg = _small_rig(W=128, H=96, n_views=2, fov=170.0)
+    images = synth.render_frame(cfg, 0)
+    cfg.update(families_low=[synth.family((0, 0, 1), 16, 0.8, 30.0, "inverse")],
+               families_crop=[synth.family((0, 0, 1), 32, 0.8, 40.0, "inverse")],
+               params_low=synth.params(5, synth.VAR_FLOOR_U8, 60.0),
+               params_crop=synth.params(7, synth.VAR_FLOOR_U8, 80.0, 0.2, 0.3, 48, 1.1, filters=3),
+               crop=(35, 27, 61, 40))
+    mask = synth.make_mask(128, 96, 11, n_rects=2)
+    mask[:, :] = 0
+    mask[10:30, 50:90] = 1
+    for host in (False, True):
+        ref, test, stats, _ = run_multires(cfg, images, mask, host=host)
+        assert_gates(stats)
+        assert (ref["kbest"] >> 14 == 1).any() and ((ref["kbest"] >= 0) & (ref["kbest"] >> 14 == 0)).any()
