@@ -193,12 +193,12 @@ def run_ours(args, rank, local_rank, world):
     W, H = cfg["cams"][0]["width"], cfg["cams"][0]["height"]
 
     # ---- inputs: N_STAGED distinct frame sets per rank, resident on the device (and pinned on the host for e2e) ----
-    frame0 = rank * N_STAGED
+    from paper_1809_06132_b200 import shard
     host_frames, host_masks = [], []
-    for f in range(N_STAGED):
-        host_frames.append(synth.render_frame(cfg, frame0 + f))
+    for f in shard.frames_for_rank(0, N_STAGED, rank, world):
+        host_frames.append(synth.render_frame(cfg, f))
         if cfg.get("mask_seed") is not None:
-            host_masks.append(synth.make_mask(W, H, cfg["mask_seed"] + frame0 + f))
+            host_masks.append(synth.make_mask(W, H, cfg["mask_seed"] + f))
     dev_frames = [[torch.from_numpy(im).to(dev) for im in fr] for fr in host_frames]
     dev_masks = [torch.from_numpy(m).to(dev) for m in host_masks] or [None] * N_STAGED
     rig = fsw.Rig(cfg["cams"], cfg["ref_index"])
@@ -282,13 +282,7 @@ def run_ours(args, rank, local_rank, world):
     launches += launches_per_step * e2e_steps
 
     # ---- max over ranks ----------------------------------------------------------------------------------------------
-    t = torch.tensor([ms_total, ms_e2e], dtype=torch.float64, device=dev)
-    ev = torch.tensor([evals_total], dtype=torch.float64, device=dev)
-    if dist is not None:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        dist.all_reduce(ev, op=dist.ReduceOp.SUM)
-    ms_total, ms_e2e = float(t[0]), float(t[1])
-    evals_all = float(ev[0])
+    (ms_total, ms_e2e), (evals_all,) = shard.reduce_timing([ms_total, ms_e2e], [evals_total], dev)
 
     if rank == 0:
         fp32_tflops, _ = fsw.measure_fp32_peak(local_rank)
