@@ -41,7 +41,7 @@ extern "C" {
 #endif
 
 #define FSW_VERSION_MAJOR 0
-#define FSW_VERSION_MINOR 1
+#define FSW_VERSION_MINOR 2
 
 /* status codes */
 #define FSW_OK 0
@@ -56,6 +56,7 @@ extern "C" {
 #define FSW_MAX_PLANES 1024
 #define FSW_MAX_FAMILIES 8
 #define FSW_MAX_WINDOW 15
+#define FSW_MAX_BATCH 256 /* frame sets per fsw_compute_depth_batch call */
 
 /* pixel types of input images */
 #define FSW_U8 0  /* uint8 grey levels 0..255 ("gray scale images") */
@@ -191,8 +192,9 @@ int32_t fsw_planeset_size(const fsw_planeset* ps, int32_t* n_planes);
 int32_t fsw_planeset_table(const fsw_planeset* ps, double* s, double* d, int32_t* family);
 
 /* ---- context (needs a CUDA device) ---------------------------------------- */
-/* Owns device-side scratch (footprint-packed view images, half-resolution images and maps, counters).  Scratch is
- * allocated lazily and reused; no hidden streams: all work is enqueued on the stream given to each call. */
+/* Owns device-side scratch (footprint images of the views, half-resolution images and maps, tile schedule, work
+ * queue, counters).  Scratch is allocated lazily and reused, so one context serves one stream at a time; no hidden
+ * streams: all work is enqueued on the stream given to each call. */
 int32_t fsw_context_create(const fsw_rig* rig, int32_t cuda_device, fsw_context** out);
 int32_t fsw_context_destroy(fsw_context* ctx);
 
@@ -207,6 +209,21 @@ int32_t fsw_compute_depth(fsw_context* ctx, const fsw_planeset* planes, const fs
                           const fsw_image* images, const uint8_t* mask, size_t mask_pitch,
                           const fsw_depth_out* out, void* cuda_stream);
 
+/* ---- depth for a batch of independent frame sets ---------------------------- */
+/* The same computation as fsw_compute_depth for n_sets synchronized frame sets of the same rig (one
+ * frame set per timestamp; the sets are independent given the rig and the plane set), enqueued as ONE sweep launch
+ * whose persistent thread blocks draw (frame set, tile) work items from a common queue, so that the tiles of one
+ * frame set fill the tail of another.  Results are identical to n_sets separate fsw_compute_depth calls.
+ * images: host array of n_sets * n_cams descriptors, set-major (images[s * n_cams + c]), device pointers.
+ * masks: host array of n_sets device pointers (each nullable), or NULL for no masks; one mask_pitch for all.
+ * outs: host array of n_sets output descriptors (device pointers; the sets must not alias each other).
+ * 1 <= n_sets <= FSW_MAX_BATCH.  The context's footprint scratch grows to n_sets frame sets (16 bytes per view
+ * pixel).  params->debug_cost_volume must be NULL unless n_sets == 1.  Asynchronous like fsw_compute_depth.
+ * fsw_get_last_counters then reports totals over the batch. */
+int32_t fsw_compute_depth_batch(fsw_context* ctx, const fsw_planeset* planes, const fsw_sweep_params* params,
+                                int32_t n_sets, const fsw_image* images, const uint8_t* const* masks, size_t mask_pitch,
+                                const fsw_depth_out* outs, void* cuda_stream);
+
 /* Two-scale strategy of PAPER.md:88-90: every image is 2x2-box downsampled and swept over the whole field of view
  * with planes_low / params_low (intrinsics f/2, c' = (c-0.5)/2); the result is upsampled (nearest neighbour); the
  * full-resolution images are swept inside `crop` with planes_crop / params_crop; inside the crop the full-resolution
@@ -217,12 +234,15 @@ int32_t fsw_compute_depth_multires(fsw_context* ctx, const fsw_planeset* planes_
                                    fsw_rect crop, const fsw_image* images, const uint8_t* mask, size_t mask_pitch,
                                    const fsw_depth_out* out, void* cuda_stream);
 
-/* Same two calls with HOST buffers: images[i].data, mask and every pointer of `out` are host memory (pinned memory
+/* Same calls with HOST buffers: images[i].data, mask and every pointer of `out` are host memory (pinned memory
  * makes the copies asynchronous).  The library stages them through context-owned device buffers on cuda_stream:
  * host->device copies, the kernels, device->host copies, then synchronizes the stream before returning. */
 int32_t fsw_compute_depth_host(fsw_context* ctx, const fsw_planeset* planes, const fsw_sweep_params* params,
                                const fsw_image* images, const uint8_t* mask, size_t mask_pitch,
                                const fsw_depth_out* out, void* cuda_stream);
+int32_t fsw_compute_depth_batch_host(fsw_context* ctx, const fsw_planeset* planes, const fsw_sweep_params* params,
+                                     int32_t n_sets, const fsw_image* images, const uint8_t* const* masks,
+                                     size_t mask_pitch, const fsw_depth_out* outs, void* cuda_stream);
 int32_t fsw_compute_depth_multires_host(fsw_context* ctx, const fsw_planeset* planes_low,
                                         const fsw_planeset* planes_crop, const fsw_sweep_params* params_low,
                                         const fsw_sweep_params* params_crop, fsw_rect crop, const fsw_image* images,

@@ -27,6 +27,7 @@ EXPORTS = (
     "fsw_ground_normal_in_ref", "fsw_planeset_create", "fsw_planeset_destroy", "fsw_planeset_size",
     "fsw_planeset_table", "fsw_context_create", "fsw_context_destroy", "fsw_compute_depth",
     "fsw_compute_depth_multires", "fsw_compute_depth_host", "fsw_compute_depth_multires_host",
+    "fsw_compute_depth_batch", "fsw_compute_depth_batch_host",
     "fsw_context_set_timing", "fsw_get_last_counters", "fsw_measure_fp32_peak",
 )
 
@@ -114,6 +115,9 @@ def load_library():
     L.fsw_compute_depth.argtypes = single
     L.fsw_compute_depth_host.argtypes = single
     L.fsw_compute_depth_multires.argtypes = multi
+    batch = [vp, vp, P(CParams), i32, P(CImage), P(vp), sz, P(CDepthOut), vp]
+    L.fsw_compute_depth_batch.argtypes = batch
+    L.fsw_compute_depth_batch_host.argtypes = batch
     L.fsw_compute_depth_multires_host.argtypes = multi
     L.fsw_context_set_timing.argtypes = [vp, i32]
     L.fsw_get_last_counters.argtypes = [vp, P(CCounters)]
@@ -347,6 +351,43 @@ class Context:
         _check(fn(self.handle, planes.handle, ctypes.byref(cp), arr, mptr, mpitch, ctypes.byref(cout), stream))
         out["_keep"] = (keep, mkeep)
         return out
+
+    def compute_depth_batch(self, planes: PlaneSet, params, image_sets, masks=None, want=ALL, host=False, outs=None):
+        """fsw_compute_depth_batch / _host: n independent frame sets of the rig in one sweep launch.
+        image_sets: list of per-set image lists; masks: list (entries may be None) or None; outs: optional list of
+        caller-owned output dicts.  Returns a list of output dicts, one per frame set."""
+        torch = _torch()
+        L = load_library()
+        n, nc = len(image_sets), self.rig.n_cams
+        arr = (CImage * (n * nc))()
+        keep = []
+        for s, images in enumerate(image_sets):
+            a, k = self._images(images, host)
+            for c in range(nc):
+                arr[s * nc + c] = a[c]
+            keep.append(k)
+        marr, mpitch = None, 0
+        if masks is not None and any(m is not None for m in masks):
+            marr = (ctypes.c_void_p * n)()
+            for s, m in enumerate(masks):
+                ptr, pitch, mk = self._mask(m, host)
+                marr[s] = ptr
+                keep.append(mk)
+                if ptr:
+                    assert mpitch in (0, pitch), "all masks of a batch share one pitch"
+                    mpitch = pitch
+        couts = (CDepthOut * n)()
+        results = []
+        for s in range(n):
+            c, o = self._outputs(host, want, None if outs is None else outs[s])
+            couts[s] = c
+            results.append(o)
+        cp = make_params(params)
+        stream = torch.cuda.current_stream(self.device).cuda_stream
+        fn = L.fsw_compute_depth_batch_host if host else L.fsw_compute_depth_batch
+        _check(fn(self.handle, planes.handle, ctypes.byref(cp), n, arr, marr, mpitch, couts, stream))
+        results[0]["_keep"] = keep
+        return results
 
     def compute_depth_multires(self, planes_low: PlaneSet, planes_crop: PlaneSet, params_low, params_crop, crop,
                                images, mask=None, want=ALL, host=False, out=None):

@@ -8,14 +8,16 @@
 #include <cstdio>
 #include <cstring>
 #include <new>
+#include <algorithm>
 #include <vector>
 
 #include "fsw_internal.h"
 
 /* per-window launchers, one object file each (fsw_sweep_inst.cu) */
-#define FSW_DECL_WIN(w)                                                               \
-    cudaError_t fsw_launch_sweep_w##w(const FswSweepArgs& args, int variant, cudaStream_t stream); \
-    cudaError_t fsw_prepare_sweep_w##w();
+#define FSW_DECL_WIN(w)                                                                                  \
+    cudaError_t fsw_launch_sweep_w##w(const FswSweepArgs& args, int variant, int grid, cudaStream_t stream); \
+    cudaError_t fsw_prepare_sweep_w##w();                                                                    \
+    FswSweepGeometry fsw_geometry_sweep_w##w(int n_views);
 FSW_DECL_WIN(3) FSW_DECL_WIN(5) FSW_DECL_WIN(7) FSW_DECL_WIN(9) FSW_DECL_WIN(11) FSW_DECL_WIN(13) FSW_DECL_WIN(15)
 #undef FSW_DECL_WIN
 
@@ -94,21 +96,38 @@ struct fsw_planeset {
     std::vector<int32_t> family;
 };
 
+/* scheduling order of the tiles of one (image size, tile shape, principal point) combination, on the device */
+struct TileOrder {
+    int32_t W, H, tw, th;
+    float cx, cy;
+    int32_t n_tiles_x, n_tiles;
+    DevBuf dev;
+};
+
+/* words of the control block: [0] work queue of the sweep kernel, [2..9] four 64-bit counters */
+#define FSW_CTRL_WORDS 10
+
 struct fsw_context {
     fsw_rig rig;
     int32_t device;
-    DevBuf foot[FSW_MAX_CAMERAS];  /* footprint-packed 8-bit views */
+    int32_t n_sm = 0;
+    std::vector<DevBuf> foot;      /* footprint images of the views: [set slot][camera] */
     DevBuf half[FSW_MAX_CAMERAS];  /* half-resolution float images */
+    DevBuf half_foot[FSW_MAX_CAMERAS];
     DevBuf lo_depth, lo_c1, lo_c2, lo_k;
-    DevBuf counters;               /* 4 x uint64 */
-    /* staging for the *_host calls */
-    DevBuf st_img[FSW_MAX_CAMERAS], st_mask, st_depth, st_c1, st_c2, st_k, st_reason;
+    DevBuf ctrl;                   /* FSW_CTRL_WORDS x uint32 */
+    DevBuf sets_dev;               /* FswSetPtrs of a batch */
+    std::vector<TileOrder*> orders;
+    /* staging for the *_host calls: [set slot] */
+    std::vector<DevBuf> st_img, st_mask, st_depth, st_c1, st_c2, st_k, st_reason;
     cudaStream_t last_stream = nullptr;
     int64_t last_launches = 0;
     bool timing = false, timed = false;
     cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr}; /* [0,1] around the (crop) sweep, [2,3] around the low sweep */
     int n_timed = 0;
     bool prepared[FSW_MAX_WINDOW + 1] = {false};
+    unsigned int* queue() { return (unsigned int*)ctrl.p; }
+    unsigned long long* counters() { return (unsigned long long*)((unsigned int*)ctrl.p + 2); }
 };
 
 namespace {
@@ -171,11 +190,28 @@ FswDevCam dev_cam(const fsw_camera& c, bool half) {
     d.fx = (float)fx; d.fy = (float)fy; d.cx = (float)cx; d.cy = (float)cy; d.xi = (float)c.xi;
     d.k1 = (float)c.k1; d.k2 = (float)c.k2; d.p1 = (float)c.p1; d.p2 = (float)c.p2;
     d.cos_fov = (float)std::cos(0.5 * c.fov_max_deg * M_PI / 180.0);
+    d.cos_fov_xi = (float)(std::cos(0.5 * c.fov_max_deg * M_PI / 180.0) + c.xi);
     d.W = W; d.H = H;
     if (c.k1 == 0.0 && c.k2 == 0.0 && c.p1 == 0.0 && c.p2 == 0.0) d.dist_mode = FSW_DIST_NONE;
     else if (c.k2 == 0.0 && c.p1 == 0.0 && c.p2 == 0.0) d.dist_mode = FSW_DIST_K1;
     else d.dist_mode = FSW_DIST_FULL;
     return d;
+}
+
+/* Squared distorted normalised radius of the edge of the field of view, with a 2 % margin: a reference pixel whose
+ * normalised coordinates lie beyond it cannot be inside the FOV, so tiles entirely beyond it skip S1.  Only when
+ * the bound is provable: radial-only distortion, monotone over the FOV (checked at rig creation), finite edge. */
+float ref_rd2_bound(const fsw_camera& c) {
+    if (c.p1 != 0.0 || c.p2 != 0.0) return INFINITY;
+    const double th = 0.5 * c.fov_max_deg * M_PI / 180.0;
+    const double den = std::cos(th) + c.xi;
+    if (!(den > 1e-3)) return INFINITY;
+    const double ru = std::sin(th) / den;
+    if (c.xi > 1.0 && std::cos(th) < -1.0 / c.xi) return INFINITY; /* rho_u(theta) is no longer monotone there */
+    const double r2 = ru * ru;
+    const double rd = ru * (1.0 + c.k1 * r2 + c.k2 * r2 * r2) * 1.02;
+    if (!(rd > 0.0) || !std::isfinite(rd)) return INFINITY;
+    return (float)(rd * rd);
 }
 
 int32_t check_params(const fsw_sweep_params* p, const char* name) {
@@ -222,6 +258,7 @@ int32_t fill_args(FswSweepArgs& a, const fsw_rig& rig, const fsw_planeset& ps, c
     std::memset(&a, 0, sizeof(a));
     const fsw_camera& ref = rig.cams[rig.ref_index];
     a.ref = dev_cam(ref, half);
+    a.ref_rd2_max = ref_rd2_bound(ref); /* normalised coordinates: the same at both resolutions */
     a.n_views = 0;
     for (int c = 0; c < rig.n_cams; ++c) {
         if (c == rig.ref_index) continue;
@@ -262,12 +299,12 @@ int32_t fill_args(FswSweepArgs& a, const fsw_rig& rig, const fsw_planeset& ps, c
     a.depth_kind = p.depth_kind;
     a.horizon_row = p.horizon_row;
     a.alpha_upper = p.alpha_upper; a.alpha_lower = p.alpha_lower; a.beta = p.beta;
-    const double n2 = (double)p.window * p.window * (double)p.window * p.window;
-    const double fl = (double)p.var_floor * n2;
+    /* the kernel compares (N var_a)(N var_b) with (var_floor N)^2, N = window^2 */
+    const double fl = (double)p.var_floor * (double)p.window * (double)p.window;
     a.floor2 = (float)(fl * fl);
     if (!(a.floor2 > 0.f)) a.floor2 = 1e-30f; /* keeps the reciprocal square root finite on flat windows */
     a.inv_range_max = 1.f / p.range_max;
-    a.debug_cost = p.debug_cost_volume;
+    a.n_sets = 1;
     return FSW_OK;
 }
 
@@ -287,74 +324,163 @@ cudaError_t prepare_window(fsw_context* ctx, int w) {
     return e;
 }
 
+FswSweepGeometry window_geometry(int w, int n_views) {
+    switch (w) {
+        case 3: return fsw_geometry_sweep_w3(n_views);
+        case 5: return fsw_geometry_sweep_w5(n_views);
+        case 7: return fsw_geometry_sweep_w7(n_views);
+        case 9: return fsw_geometry_sweep_w9(n_views);
+        case 11: return fsw_geometry_sweep_w11(n_views);
+        case 13: return fsw_geometry_sweep_w13(n_views);
+        default: return fsw_geometry_sweep_w15(n_views);
+    }
+}
+
 /* picks the kernel variant the views allow (see fsw_sweep.cuh) */
 int pick_variant(const FswSweepArgs& a) {
-    bool ident = true, k1only = true, all_u8 = true, all_f32 = true;
+    bool fast = true;
     for (int v = 0; v < a.n_views; ++v) {
-        ident = ident && a.views[v].ident_R;
-        k1only = k1only && a.views[v].cam.dist_mode != FSW_DIST_FULL;
-        k1only = k1only && (a.views[v].cam.cos_fov + a.views[v].cam.xi >= 1e-3f); /* lets the kernel drop the den test */
-        all_u8 = all_u8 && a.views[v].pix_mode == FSW_PIX_FOOT_U8;
-        all_f32 = all_f32 && a.views[v].pix_mode == FSW_PIX_F32;
+        fast = fast && a.views[v].ident_R;
+        fast = fast && a.views[v].cam.dist_mode != FSW_DIST_FULL;
+        fast = fast && (a.views[v].cam.cos_fov_xi >= 1e-3f); /* lets the kernel drop the denominator test */
     }
-    if (ident && k1only && all_u8) return 1;
-    if (ident && k1only && all_f32) return 2;
-    return 0;
+    return fast ? 1 : 0;
 }
 
-cudaError_t launch_window(const FswSweepArgs& a, int w, cudaStream_t s) {
-    const int var = pick_variant(a);
-    switch (w) {
-        case 3: return fsw_launch_sweep_w3(a, var, s);
-        case 5: return fsw_launch_sweep_w5(a, var, s);
-        case 7: return fsw_launch_sweep_w7(a, var, s);
-        case 9: return fsw_launch_sweep_w9(a, var, s);
-        case 11: return fsw_launch_sweep_w11(a, var, s);
-        case 13: return fsw_launch_sweep_w13(a, var, s);
-        case 15: return fsw_launch_sweep_w15(a, var, s);
-    }
-    return cudaErrorInvalidValue;
-}
-
-/* makes the device representation of every matching view: 8-bit images are footprint-packed into context scratch
- * (one launch for all of them), float images are used in place */
-int32_t stage_views(fsw_context* ctx, const fsw_image* images, FswSweepArgs& a, cudaStream_t stream, bool zero_counters,
-                    bool* zeroed) {
-    const fsw_rig& rig = ctx->rig;
-    FswPackArgs pk;
-    std::memset(&pk, 0, sizeof(pk));
-    int vi = 0;
-    for (int c = 0; c < rig.n_cams; ++c) {
-        if (c == rig.ref_index) continue;
-        FswDevView& v = a.views[vi++];
-        const int W = rig.cams[c].width, H = rig.cams[c].height;
-        if (images[c].dtype == FSW_U8) {
-            FSW_CUDA(ctx->foot[c].reserve((size_t)W * H * 4));
-            pk.src[pk.n] = (const uint8_t*)images[c].data;
-            pk.src_pitch[pk.n] = (int64_t)images[c].pitch_bytes;
-            pk.dst[pk.n] = (uint32_t*)ctx->foot[c].p;
-            pk.W[pk.n] = W; pk.H[pk.n] = H;
-            pk.n++;
-            v.pix_mode = FSW_PIX_FOOT_U8;
-            v.img = ctx->foot[c].p;
-            v.pitch_elems = W;
-        } else {
-            v.pix_mode = FSW_PIX_F32;
-            v.img = images[c].data;
-            v.pitch_elems = (int64_t)(images[c].pitch_bytes / 4);
+/* Scheduling order of the tiles (S0): nearest to the principal point first, lower image half before the upper
+ * half at equal distance (its rays also face ground-parallel planes).  Tiles inside the image circle are the
+ * expensive ones; the cheap ones (outside the field of view) fill the tail of the persistent grid. */
+int32_t get_tile_order(fsw_context* ctx, const FswDevCam& ref, const FswSweepGeometry& g, const TileOrder** out) {
+    for (TileOrder* t : ctx->orders)
+        if (t->W == ref.W && t->H == ref.H && t->tw == g.tile_w && t->th == g.tile_h && t->cx == ref.cx && t->cy == ref.cy) {
+            *out = t;
+            return FSW_OK;
         }
+    TileOrder* t = new (std::nothrow) TileOrder;
+    if (!t) return fail(FSW_E_NOMEM, "tile order: out of memory");
+    t->W = ref.W; t->H = ref.H; t->tw = g.tile_w; t->th = g.tile_h; t->cx = ref.cx; t->cy = ref.cy;
+    t->n_tiles_x = (ref.W + g.tile_w - 1) / g.tile_w;
+    const int nty = (ref.H + g.tile_h - 1) / g.tile_h;
+    t->n_tiles = t->n_tiles_x * nty;
+    std::vector<std::pair<float, int32_t>> key((size_t)t->n_tiles);
+    for (int ty = 0; ty < nty; ++ty)
+        for (int tx = 0; tx < t->n_tiles_x; ++tx) {
+            float dx = ((float)tx + 0.5f) * g.tile_w - 0.5f - ref.cx, dy = ((float)ty + 0.5f) * g.tile_h - 0.5f - ref.cy;
+            float r = std::sqrt(dx * dx + dy * dy) - (dy > 0.f ? 0.25f * g.tile_h : 0.f);
+            key[(size_t)ty * t->n_tiles_x + tx] = std::make_pair(r, (int32_t)(ty * t->n_tiles_x + tx));
+        }
+    std::stable_sort(key.begin(), key.end());
+    std::vector<int32_t> order((size_t)t->n_tiles);
+    for (int i = 0; i < t->n_tiles; ++i) order[i] = key[i].second;
+    cudaError_t e = t->dev.reserve(sizeof(int32_t) * (size_t)t->n_tiles);
+    if (e == cudaSuccess) e = cudaMemcpy(t->dev.p, order.data(), sizeof(int32_t) * (size_t)t->n_tiles, cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) {
+        t->dev.release();
+        delete t;
+        return cuda_fail(e, "tile order upload");
     }
-    *zeroed = false;
-    if (pk.n > 0) {
-        pk.counters_to_zero = zero_counters ? (unsigned long long*)ctx->counters.p : nullptr;
-        FSW_CUDA(fsw_launch_pack_footprints(pk, stream));
-        ctx->last_launches++;
-        *zeroed = zero_counters;
-    }
+    ctx->orders.push_back(t);
+    *out = t;
     return FSW_OK;
 }
 
-void set_outputs(FswSweepArgs& a, const fsw_depth_out* out, const uint8_t* mask, size_t mask_pitch) {
+/* enqueues the sweep kernel for a.n_sets frame sets (a.set0 / a.sets filled by the caller); the queue word must be
+ * zero when the kernel starts (the pack launch before it clears it) */
+int32_t launch_sweep(fsw_context* ctx, FswSweepArgs& a, int w, cudaStream_t s) {
+    const FswSweepGeometry g = window_geometry(w, a.n_views);
+    const TileOrder* order = nullptr;
+    int32_t rc = get_tile_order(ctx, a.ref, g, &order);
+    if (rc != FSW_OK) return rc;
+    a.tile_order = (const int32_t*)order->dev.p;
+    a.n_tiles_x = order->n_tiles_x;
+    a.n_tiles = order->n_tiles;
+    a.queue = ctx->queue();
+    a.counters = ctx->counters();
+    const long long items = (long long)a.n_tiles * a.n_sets;
+    const long long slots = (long long)ctx->n_sm * g.ctas_per_sm;
+    const int grid = (int)(items < slots ? items : slots);
+    const int var = pick_variant(a);
+    cudaError_t e = cudaErrorInvalidValue;
+    switch (w) {
+        case 3: e = fsw_launch_sweep_w3(a, var, grid, s); break;
+        case 5: e = fsw_launch_sweep_w5(a, var, grid, s); break;
+        case 7: e = fsw_launch_sweep_w7(a, var, grid, s); break;
+        case 9: e = fsw_launch_sweep_w9(a, var, grid, s); break;
+        case 11: e = fsw_launch_sweep_w11(a, var, grid, s); break;
+        case 13: e = fsw_launch_sweep_w13(a, var, grid, s); break;
+        case 15: e = fsw_launch_sweep_w15(a, var, grid, s); break;
+    }
+    if (e != cudaSuccess) return cuda_fail(e, "sweep kernel launch");
+    ctx->last_launches++;
+    return FSW_OK;
+}
+
+/* S4 staging: builds the footprint image of every matching view of n_sets frame sets (images[set * n_cams + cam]) in
+ * context scratch and records the pointers in sets[]; the first pack launch also clears the work queue (and the
+ * counters if asked).  half = the images are the context's half-resolution float images. */
+int32_t stage_views(fsw_context* ctx, const fsw_image* images, int n_sets, bool half, FswSetPtrs* sets,
+                    cudaStream_t stream, bool zero_counters) {
+    const fsw_rig& rig = ctx->rig;
+    if (!half && ctx->foot.size() < (size_t)n_sets * FSW_MAX_CAMERAS) ctx->foot.resize((size_t)n_sets * FSW_MAX_CAMERAS);
+    bool first = true;
+    /* one launch per camera size (all views of a rig usually share one) and per FSW_PACK_MAX images */
+    std::vector<bool> done((size_t)rig.n_cams, false);
+    for (int c0 = 0; c0 < rig.n_cams; ++c0) {
+        if (c0 == rig.ref_index || done[c0]) continue;
+        const int W = half ? rig.cams[c0].width / 2 : rig.cams[c0].width;
+        const int H = half ? rig.cams[c0].height / 2 : rig.cams[c0].height;
+        FswPackArgs pk;
+        std::memset(&pk, 0, sizeof(pk));
+        pk.W = W; pk.H = H;
+        auto flush = [&]() -> int32_t {
+            if (pk.n == 0) return FSW_OK;
+            if (first) {
+                pk.words_to_zero = (unsigned int*)ctx->ctrl.p;
+                pk.n_words_to_zero = zero_counters ? FSW_CTRL_WORDS : 1;
+                first = false;
+            } else {
+                pk.words_to_zero = nullptr;
+                pk.n_words_to_zero = 0;
+            }
+            FSW_CUDA(fsw_launch_pack_footprints(pk, stream));
+            ctx->last_launches++;
+            pk.n = 0;
+            return FSW_OK;
+        };
+        for (int c = c0; c < rig.n_cams; ++c) {
+            if (c == rig.ref_index || done[c]) continue;
+            const int Wc = half ? rig.cams[c].width / 2 : rig.cams[c].width;
+            const int Hc = half ? rig.cams[c].height / 2 : rig.cams[c].height;
+            if (Wc != W || Hc != H) continue;
+            done[c] = true;
+            int vi = c < rig.ref_index ? c : c - 1; /* view index = camera order without the reference */
+            for (int s = 0; s < n_sets; ++s) {
+                DevBuf& fb = half ? ctx->half_foot[c] : ctx->foot[(size_t)s * FSW_MAX_CAMERAS + c];
+                FSW_CUDA(fb.reserve((size_t)W * H * sizeof(float4)));
+                if (half) {
+                    pk.src[pk.n] = ctx->half[c].p; pk.src_pitch[pk.n] = (int64_t)W * 4; pk.dtype[pk.n] = FSW_F32;
+                } else {
+                    const fsw_image& im = images[(size_t)s * rig.n_cams + c];
+                    pk.src[pk.n] = im.data; pk.src_pitch[pk.n] = (int64_t)im.pitch_bytes; pk.dtype[pk.n] = im.dtype;
+                }
+                pk.dst[pk.n] = (float4*)fb.p;
+                sets[s].foot[vi] = (const float4*)fb.p;
+                pk.n++;
+                if (pk.n == FSW_PACK_MAX) {
+                    int32_t rc = flush();
+                    if (rc != FSW_OK) return rc;
+                }
+            }
+        }
+        int32_t rc = flush();
+        if (rc != FSW_OK) return rc;
+    }
+    if (first) /* cannot happen (a rig has at least one view), but never start a sweep with a dirty queue */
+        FSW_CUDA(cudaMemsetAsync(ctx->ctrl.p, 0, (zero_counters ? FSW_CTRL_WORDS : 1) * sizeof(unsigned int), stream));
+    return FSW_OK;
+}
+
+void set_outputs(FswSetPtrs& a, const fsw_depth_out* out, const uint8_t* mask, size_t mask_pitch) {
     a.mask = mask; a.mask_pitch = (int64_t)mask_pitch;
     a.out_depth = out->depth; a.out_depth_pitch = (int64_t)out->depth_pitch;
     a.out_c1 = out->best_cost; a.out_c1_pitch = (int64_t)out->best_cost_pitch;
@@ -498,10 +624,11 @@ int32_t fsw_context_create(const fsw_rig* rig, int32_t cuda_device, fsw_context*
     if (!ctx) return fail(FSW_E_NOMEM, "fsw_context_create: out of memory");
     ctx->rig = *rig;
     ctx->device = cuda_device;
+    ctx->n_sm = prop.multiProcessorCount;
     DeviceGuard g;
     e = g.enter(cuda_device);
-    if (e == cudaSuccess) e = ctx->counters.reserve(4 * sizeof(unsigned long long));
-    if (e == cudaSuccess) e = cudaMemset(ctx->counters.p, 0, 4 * sizeof(unsigned long long));
+    if (e == cudaSuccess) e = ctx->ctrl.reserve(FSW_CTRL_WORDS * sizeof(unsigned int));
+    if (e == cudaSuccess) e = cudaMemset(ctx->ctrl.p, 0, FSW_CTRL_WORDS * sizeof(unsigned int));
     if (e != cudaSuccess) {
         delete ctx;
         return cuda_fail(e, "fsw_context_create");
@@ -515,24 +642,37 @@ int32_t fsw_context_destroy(fsw_context* ctx) {
     DeviceGuard g;
     g.enter(ctx->device);
     for (int c = 0; c < FSW_MAX_CAMERAS; ++c) {
-        ctx->foot[c].release(); ctx->half[c].release(); ctx->st_img[c].release();
+        ctx->half[c].release(); ctx->half_foot[c].release();
     }
-    ctx->lo_depth.release(); ctx->lo_c1.release(); ctx->lo_c2.release(); ctx->lo_k.release(); ctx->counters.release();
+    for (std::vector<DevBuf>* v : {&ctx->foot, &ctx->st_img, &ctx->st_mask, &ctx->st_depth, &ctx->st_c1, &ctx->st_c2, &ctx->st_k, &ctx->st_reason})
+        for (DevBuf& b : *v) b.release();
+    ctx->lo_depth.release(); ctx->lo_c1.release(); ctx->lo_c2.release(); ctx->lo_k.release();
+    ctx->ctrl.release(); ctx->sets_dev.release();
+    for (TileOrder* t : ctx->orders) {
+        t->dev.release();
+        delete t;
+    }
     for (int i = 0; i < 4; ++i)
         if (ctx->ev[i]) cudaEventDestroy(ctx->ev[i]);
-    ctx->st_mask.release(); ctx->st_depth.release(); ctx->st_c1.release(); ctx->st_c2.release(); ctx->st_k.release(); ctx->st_reason.release();
     delete ctx;
     return FSW_OK;
 }
 
-int32_t fsw_compute_depth(fsw_context* ctx, const fsw_planeset* planes, const fsw_sweep_params* params,
-                          const fsw_image* images, const uint8_t* mask, size_t mask_pitch,
-                          const fsw_depth_out* out, void* cuda_stream) {
-    if (!ctx || !planes) return fail(FSW_E_INVALID_ARG, "fsw_compute_depth: null context or plane set");
+/* the single-resolution path for n_sets frame sets: pack launch(es) + one sweep launch */
+static int32_t run_sets(fsw_context* ctx, const fsw_planeset* planes, const fsw_sweep_params* params, int32_t n_sets,
+                        const fsw_image* images, const uint8_t* const* masks, size_t mask_pitch,
+                        const fsw_depth_out* outs, void* cuda_stream, const char* who) {
+    if (!ctx || !planes) return fail(FSW_E_INVALID_ARG, "%s: null context or plane set", who);
+    if (n_sets < 1 || n_sets > FSW_MAX_BATCH) return fail(FSW_E_INVALID_ARG, "%s: n_sets=%d must be in 1..%d", who, n_sets, FSW_MAX_BATCH);
     int32_t rc;
     if ((rc = check_params(params, "params")) != FSW_OK) return rc;
-    if ((rc = check_images(ctx->rig, images)) != FSW_OK) return rc;
-    if ((rc = check_out(ctx->rig, out, mask, mask_pitch)) != FSW_OK) return rc;
+    if (!images || !outs) return fail(FSW_E_INVALID_ARG, "%s: null images or outputs", who);
+    const fsw_rig& rig = ctx->rig;
+    for (int s = 0; s < n_sets; ++s) {
+        if ((rc = check_images(rig, images + (size_t)s * rig.n_cams)) != FSW_OK) return rc;
+        if ((rc = check_out(rig, &outs[s], masks ? masks[s] : nullptr, mask_pitch)) != FSW_OK) return rc;
+    }
+    if (params->debug_cost_volume && n_sets > 1) return fail(FSW_E_UNSUPPORTED, "%s: debug_cost_volume needs n_sets == 1", who);
     cudaStream_t stream = (cudaStream_t)cuda_stream;
     DeviceGuard g;
     FSW_CUDA(g.enter(ctx->device));
@@ -541,21 +681,43 @@ int32_t fsw_compute_depth(fsw_context* ctx, const fsw_planeset* planes, const fs
     ctx->last_launches = 0;
 
     FswSweepArgs a;
-    fill_args(a, ctx->rig, *planes, *params, false);
-    const fsw_image& ri = images[ctx->rig.ref_index];
-    a.ref_img = ri.data; a.ref_pitch_bytes = (int64_t)ri.pitch_bytes; a.ref_dtype = ri.dtype;
-    bool zeroed = false;
-    if ((rc = stage_views(ctx, images, a, stream, true, &zeroed)) != FSW_OK) return rc;
-    if (!zeroed) FSW_CUDA(cudaMemsetAsync(ctx->counters.p, 0, 4 * sizeof(unsigned long long), stream));
-    set_outputs(a, out, mask, mask_pitch);
-    a.counters = (unsigned long long*)ctx->counters.p;
+    fill_args(a, rig, *planes, *params, false);
+    std::vector<FswSetPtrs> sets((size_t)n_sets);
+    std::memset(sets.data(), 0, sizeof(FswSetPtrs) * (size_t)n_sets);
+    for (int s = 0; s < n_sets; ++s) {
+        const fsw_image& ri = images[(size_t)s * rig.n_cams + rig.ref_index];
+        sets[s].ref_img = ri.data; sets[s].ref_pitch_bytes = (int64_t)ri.pitch_bytes; sets[s].ref_dtype = ri.dtype;
+        sets[s].debug_cost = params->debug_cost_volume;
+        set_outputs(sets[s], &outs[s], masks ? masks[s] : nullptr, mask_pitch);
+    }
+    if ((rc = stage_views(ctx, images, n_sets, false, sets.data(), stream, true)) != FSW_OK) return rc;
+    a.n_sets = n_sets;
+    a.set0 = sets[0];
+    if (n_sets > 1) {
+        FSW_CUDA(ctx->sets_dev.reserve(sizeof(FswSetPtrs) * (size_t)n_sets));
+        /* pageable source: the runtime stages it before returning, so the vector may die with this call */
+        FSW_CUDA(cudaMemcpyAsync(ctx->sets_dev.p, sets.data(), sizeof(FswSetPtrs) * (size_t)n_sets, cudaMemcpyHostToDevice, stream));
+        a.sets = (const FswSetPtrs*)ctx->sets_dev.p;
+    }
     a.count_pixels = 1;
     ctx->n_timed = 0;
     if (ctx->timing) FSW_CUDA(cudaEventRecord(ctx->ev[0], stream));
-    FSW_CUDA(launch_window(a, params->window, stream));
+    if ((rc = launch_sweep(ctx, a, params->window, stream)) != FSW_OK) return rc;
     if (ctx->timing) { FSW_CUDA(cudaEventRecord(ctx->ev[1], stream)); ctx->n_timed = 1; }
-    ctx->last_launches++;
     return FSW_OK;
+}
+
+int32_t fsw_compute_depth(fsw_context* ctx, const fsw_planeset* planes, const fsw_sweep_params* params,
+                          const fsw_image* images, const uint8_t* mask, size_t mask_pitch,
+                          const fsw_depth_out* out, void* cuda_stream) {
+    const uint8_t* masks[1] = {mask};
+    return run_sets(ctx, planes, params, 1, images, mask ? masks : nullptr, mask_pitch, out, cuda_stream, "fsw_compute_depth");
+}
+
+int32_t fsw_compute_depth_batch(fsw_context* ctx, const fsw_planeset* planes, const fsw_sweep_params* params,
+                                int32_t n_sets, const fsw_image* images, const uint8_t* const* masks, size_t mask_pitch,
+                                const fsw_depth_out* outs, void* cuda_stream) {
+    return run_sets(ctx, planes, params, n_sets, images, masks, mask_pitch, outs, cuda_stream, "fsw_compute_depth_batch");
 }
 
 int32_t fsw_compute_depth_multires(fsw_context* ctx, const fsw_planeset* planes_low, const fsw_planeset* planes_crop,
@@ -592,7 +754,6 @@ int32_t fsw_compute_depth_multires(fsw_context* ctx, const fsw_planeset* planes_
         dn.src[c] = images[c].data; dn.src_pitch[c] = (int64_t)images[c].pitch_bytes; dn.dtype[c] = images[c].dtype;
         dn.dst[c] = (float*)ctx->half[c].p; dn.W[c] = W; dn.H[c] = H;
     }
-    dn.counters_to_zero = (unsigned long long*)ctx->counters.p;
     FSW_CUDA(fsw_launch_downsample(dn, stream));
     ctx->last_launches++;
 
@@ -606,92 +767,108 @@ int32_t fsw_compute_depth_multires(fsw_context* ctx, const fsw_planeset* planes_
     fsw_sweep_params pl = *params_low;
     pl.filters_enabled = 0; /* filters run after the merge (reading Q20) */
     fill_args(a, rig, *planes_low, pl, true);
-    a.ref_img = ctx->half[rig.ref_index].p; a.ref_pitch_bytes = (int64_t)LW * 4; a.ref_dtype = FSW_F32;
-    {
-        int vi = 0;
-        for (int c = 0; c < rig.n_cams; ++c) {
-            if (c == rig.ref_index) continue;
-            FswDevView& v = a.views[vi++];
-            v.pix_mode = FSW_PIX_F32; v.img = ctx->half[c].p; v.pitch_elems = rig.cams[c].width / 2;
-        }
-    }
-    a.out_depth = (float*)ctx->lo_depth.p; a.out_depth_pitch = (int64_t)LW * 4;
-    a.out_c1 = (float*)ctx->lo_c1.p; a.out_c1_pitch = (int64_t)LW * 4;
-    a.out_c2 = (float*)ctx->lo_c2.p; a.out_c2_pitch = (int64_t)LW * 4;
-    a.out_k = (int16_t*)ctx->lo_k.p; a.out_k_pitch = (int64_t)LW * 2;
-    a.counters = (unsigned long long*)ctx->counters.p;
+    FswSetPtrs lo;
+    std::memset(&lo, 0, sizeof(lo));
+    lo.ref_img = ctx->half[rig.ref_index].p; lo.ref_pitch_bytes = (int64_t)LW * 4; lo.ref_dtype = FSW_F32;
+    lo.out_depth = (float*)ctx->lo_depth.p; lo.out_depth_pitch = (int64_t)LW * 4;
+    lo.out_c1 = (float*)ctx->lo_c1.p; lo.out_c1_pitch = (int64_t)LW * 4;
+    lo.out_c2 = (float*)ctx->lo_c2.p; lo.out_c2_pitch = (int64_t)LW * 4;
+    lo.out_k = (int16_t*)ctx->lo_k.p; lo.out_k_pitch = (int64_t)LW * 2;
+    if ((rc = stage_views(ctx, nullptr, 1, true, &lo, stream, true)) != FSW_OK) return rc;
+    a.set0 = lo;
     a.count_pixels = 0;
     ctx->n_timed = 0;
     if (ctx->timing) FSW_CUDA(cudaEventRecord(ctx->ev[2], stream));
-    FSW_CUDA(launch_window(a, params_low->window, stream));
+    if ((rc = launch_sweep(ctx, a, params_low->window, stream)) != FSW_OK) return rc;
     if (ctx->timing) FSW_CUDA(cudaEventRecord(ctx->ev[3], stream));
-    ctx->last_launches++;
 
     /* S10(d)-(e) + S9 + S11: full-resolution sweep inside the crop, merged with the upsampled maps in its epilogue */
     fsw_sweep_params pc = *params_crop;
     pc.roi = crop;
     fill_args(a, rig, *planes_crop, pc, false);
+    FswSetPtrs hi;
+    std::memset(&hi, 0, sizeof(hi));
     const fsw_image& ri = images[rig.ref_index];
-    a.ref_img = ri.data; a.ref_pitch_bytes = (int64_t)ri.pitch_bytes; a.ref_dtype = ri.dtype;
-    bool zeroed = false;
-    if ((rc = stage_views(ctx, images, a, stream, false, &zeroed)) != FSW_OK) return rc;
-    set_outputs(a, out, mask, mask_pitch);
-    a.lo_depth = (const float*)ctx->lo_depth.p; a.lo_c1 = (const float*)ctx->lo_c1.p; a.lo_c2 = (const float*)ctx->lo_c2.p;
-    a.lo_k = (const int16_t*)ctx->lo_k.p; a.lo_W = LW; a.lo_H = LH;
+    hi.ref_img = ri.data; hi.ref_pitch_bytes = (int64_t)ri.pitch_bytes; hi.ref_dtype = ri.dtype;
+    set_outputs(hi, out, mask, mask_pitch);
+    hi.lo_depth = (const float*)ctx->lo_depth.p; hi.lo_c1 = (const float*)ctx->lo_c1.p; hi.lo_c2 = (const float*)ctx->lo_c2.p;
+    hi.lo_k = (const int16_t*)ctx->lo_k.p;
+    if ((rc = stage_views(ctx, images, 1, false, &hi, stream, false)) != FSW_OK) return rc;
+    a.set0 = hi;
+    a.lo_W = LW; a.lo_H = LH;
     a.index_flag = FSW_INDEX_FROM_CROP;
-    a.counters = (unsigned long long*)ctx->counters.p;
     a.count_pixels = 1;
     if (ctx->timing) FSW_CUDA(cudaEventRecord(ctx->ev[0], stream));
-    FSW_CUDA(launch_window(a, params_crop->window, stream));
+    if ((rc = launch_sweep(ctx, a, params_crop->window, stream)) != FSW_OK) return rc;
     if (ctx->timing) { FSW_CUDA(cudaEventRecord(ctx->ev[1], stream)); ctx->n_timed = 2; }
-    ctx->last_launches++;
     return FSW_OK;
 }
 
 /* ---- host-buffer variants ------------------------------------------------------------------------------------- */
 static int32_t run_host(fsw_context* ctx, bool multires, const fsw_planeset* p0, const fsw_planeset* p1,
-                        const fsw_sweep_params* q0, const fsw_sweep_params* q1, fsw_rect crop, const fsw_image* images,
-                        const uint8_t* mask, size_t mask_pitch, const fsw_depth_out* out, void* cuda_stream) {
+                        const fsw_sweep_params* q0, const fsw_sweep_params* q1, fsw_rect crop, int32_t n_sets,
+                        const fsw_image* images, const uint8_t* const* masks, size_t mask_pitch,
+                        const fsw_depth_out* outs, void* cuda_stream) {
     if (!ctx) return fail(FSW_E_INVALID_ARG, "null context");
+    if (n_sets < 1 || n_sets > FSW_MAX_BATCH) return fail(FSW_E_INVALID_ARG, "n_sets=%d must be in 1..%d", n_sets, FSW_MAX_BATCH);
+    if (!images || !outs) return fail(FSW_E_INVALID_ARG, "null images or outputs");
     int32_t rc;
-    if ((rc = check_images(ctx->rig, images)) != FSW_OK) return rc;
-    if ((rc = check_out(ctx->rig, out, mask, mask_pitch)) != FSW_OK) return rc;
+    const fsw_rig& rig = ctx->rig;
+    for (int s = 0; s < n_sets; ++s) {
+        if ((rc = check_images(rig, images + (size_t)s * rig.n_cams)) != FSW_OK) return rc;
+        if ((rc = check_out(rig, &outs[s], masks ? masks[s] : nullptr, mask_pitch)) != FSW_OK) return rc;
+    }
     cudaStream_t stream = (cudaStream_t)cuda_stream;
     DeviceGuard g;
     FSW_CUDA(g.enter(ctx->device));
-    const fsw_rig& rig = ctx->rig;
     const int W = rig.cams[rig.ref_index].width, H = rig.cams[rig.ref_index].height;
-    fsw_image dimg[FSW_MAX_CAMERAS];
-    for (int c = 0; c < rig.n_cams; ++c) {
-        const size_t es = images[c].dtype == FSW_U8 ? 1 : 4;
-        const size_t row = es * (size_t)rig.cams[c].width;
-        FSW_CUDA(ctx->st_img[c].reserve(row * rig.cams[c].height));
-        FSW_CUDA(cudaMemcpy2DAsync(ctx->st_img[c].p, row, images[c].data, images[c].pitch_bytes, row, rig.cams[c].height, cudaMemcpyHostToDevice, stream));
-        dimg[c].data = ctx->st_img[c].p; dimg[c].pitch_bytes = row; dimg[c].dtype = images[c].dtype;
+    const size_t ns = (size_t)n_sets;
+    if (ctx->st_img.size() < ns * FSW_MAX_CAMERAS) ctx->st_img.resize(ns * FSW_MAX_CAMERAS);
+    for (std::vector<DevBuf>* v : {&ctx->st_mask, &ctx->st_depth, &ctx->st_c1, &ctx->st_c2, &ctx->st_k, &ctx->st_reason})
+        if (v->size() < ns) v->resize(ns);
+    std::vector<fsw_image> dimg(ns * rig.n_cams);
+    std::vector<const uint8_t*> dmask(ns, nullptr);
+    std::vector<fsw_depth_out> dout(ns);
+    for (int s = 0; s < n_sets; ++s) {
+        for (int c = 0; c < rig.n_cams; ++c) {
+            const fsw_image& im = images[(size_t)s * rig.n_cams + c];
+            const size_t es = im.dtype == FSW_U8 ? 1 : 4;
+            const size_t row = es * (size_t)rig.cams[c].width;
+            DevBuf& b = ctx->st_img[(size_t)s * FSW_MAX_CAMERAS + c];
+            FSW_CUDA(b.reserve(row * rig.cams[c].height));
+            FSW_CUDA(cudaMemcpy2DAsync(b.p, row, im.data, im.pitch_bytes, row, rig.cams[c].height, cudaMemcpyHostToDevice, stream));
+            fsw_image& d = dimg[(size_t)s * rig.n_cams + c];
+            d.data = b.p; d.pitch_bytes = row; d.dtype = im.dtype;
+        }
+        if (masks && masks[s]) {
+            FSW_CUDA(ctx->st_mask[s].reserve((size_t)W * H));
+            FSW_CUDA(cudaMemcpy2DAsync(ctx->st_mask[s].p, W, masks[s], mask_pitch, W, H, cudaMemcpyHostToDevice, stream));
+            dmask[s] = (const uint8_t*)ctx->st_mask[s].p;
+        }
+        fsw_depth_out& o = dout[s];
+        std::memset(&o, 0, sizeof(o));
+        o.struct_size = sizeof(o);
+        FSW_CUDA(ctx->st_depth[s].reserve((size_t)W * H * 4));
+        o.depth = (float*)ctx->st_depth[s].p; o.depth_pitch = (size_t)W * 4;
+        if (outs[s].best_cost) { FSW_CUDA(ctx->st_c1[s].reserve((size_t)W * H * 4)); o.best_cost = (float*)ctx->st_c1[s].p; o.best_cost_pitch = (size_t)W * 4; }
+        if (outs[s].second_cost) { FSW_CUDA(ctx->st_c2[s].reserve((size_t)W * H * 4)); o.second_cost = (float*)ctx->st_c2[s].p; o.second_cost_pitch = (size_t)W * 4; }
+        if (outs[s].plane_index) { FSW_CUDA(ctx->st_k[s].reserve((size_t)W * H * 2)); o.plane_index = (int16_t*)ctx->st_k[s].p; o.plane_index_pitch = (size_t)W * 2; }
+        if (outs[s].valid_reason) { FSW_CUDA(ctx->st_reason[s].reserve((size_t)W * H)); o.valid_reason = (uint8_t*)ctx->st_reason[s].p; o.valid_reason_pitch = (size_t)W; }
     }
-    const uint8_t* dmask = nullptr;
-    if (mask) {
-        FSW_CUDA(ctx->st_mask.reserve((size_t)W * H));
-        FSW_CUDA(cudaMemcpy2DAsync(ctx->st_mask.p, W, mask, mask_pitch, W, H, cudaMemcpyHostToDevice, stream));
-        dmask = (const uint8_t*)ctx->st_mask.p;
-    }
-    fsw_depth_out dout;
-    std::memset(&dout, 0, sizeof(dout));
-    dout.struct_size = sizeof(dout);
-    FSW_CUDA(ctx->st_depth.reserve((size_t)W * H * 4));
-    dout.depth = (float*)ctx->st_depth.p; dout.depth_pitch = (size_t)W * 4;
-    if (out->best_cost) { FSW_CUDA(ctx->st_c1.reserve((size_t)W * H * 4)); dout.best_cost = (float*)ctx->st_c1.p; dout.best_cost_pitch = (size_t)W * 4; }
-    if (out->second_cost) { FSW_CUDA(ctx->st_c2.reserve((size_t)W * H * 4)); dout.second_cost = (float*)ctx->st_c2.p; dout.second_cost_pitch = (size_t)W * 4; }
-    if (out->plane_index) { FSW_CUDA(ctx->st_k.reserve((size_t)W * H * 2)); dout.plane_index = (int16_t*)ctx->st_k.p; dout.plane_index_pitch = (size_t)W * 2; }
-    if (out->valid_reason) { FSW_CUDA(ctx->st_reason.reserve((size_t)W * H)); dout.valid_reason = (uint8_t*)ctx->st_reason.p; dout.valid_reason_pitch = (size_t)W; }
-    if (multires) rc = fsw_compute_depth_multires(ctx, p0, p1, q0, q1, crop, dimg, dmask, (size_t)W, &dout, cuda_stream);
-    else rc = fsw_compute_depth(ctx, p0, q0, dimg, dmask, (size_t)W, &dout, cuda_stream);
+    bool any_mask = false;
+    for (int s = 0; s < n_sets; ++s) any_mask = any_mask || dmask[s] != nullptr;
+    if (multires) rc = fsw_compute_depth_multires(ctx, p0, p1, q0, q1, crop, dimg.data(), dmask[0], (size_t)W, &dout[0], cuda_stream);
+    else rc = run_sets(ctx, p0, q0, n_sets, dimg.data(), any_mask ? dmask.data() : nullptr, (size_t)W, dout.data(), cuda_stream, "fsw_compute_depth_host");
     if (rc != FSW_OK) return rc;
-    FSW_CUDA(cudaMemcpy2DAsync(out->depth, out->depth_pitch, dout.depth, dout.depth_pitch, (size_t)W * 4, H, cudaMemcpyDeviceToHost, stream));
-    if (out->best_cost) FSW_CUDA(cudaMemcpy2DAsync(out->best_cost, out->best_cost_pitch, dout.best_cost, dout.best_cost_pitch, (size_t)W * 4, H, cudaMemcpyDeviceToHost, stream));
-    if (out->second_cost) FSW_CUDA(cudaMemcpy2DAsync(out->second_cost, out->second_cost_pitch, dout.second_cost, dout.second_cost_pitch, (size_t)W * 4, H, cudaMemcpyDeviceToHost, stream));
-    if (out->plane_index) FSW_CUDA(cudaMemcpy2DAsync(out->plane_index, out->plane_index_pitch, dout.plane_index, dout.plane_index_pitch, (size_t)W * 2, H, cudaMemcpyDeviceToHost, stream));
-    if (out->valid_reason) FSW_CUDA(cudaMemcpy2DAsync(out->valid_reason, out->valid_reason_pitch, dout.valid_reason, dout.valid_reason_pitch, (size_t)W, H, cudaMemcpyDeviceToHost, stream));
+    for (int s = 0; s < n_sets; ++s) {
+        const fsw_depth_out& o = dout[s];
+        const fsw_depth_out* out = &outs[s];
+        FSW_CUDA(cudaMemcpy2DAsync(out->depth, out->depth_pitch, o.depth, o.depth_pitch, (size_t)W * 4, H, cudaMemcpyDeviceToHost, stream));
+        if (out->best_cost) FSW_CUDA(cudaMemcpy2DAsync(out->best_cost, out->best_cost_pitch, o.best_cost, o.best_cost_pitch, (size_t)W * 4, H, cudaMemcpyDeviceToHost, stream));
+        if (out->second_cost) FSW_CUDA(cudaMemcpy2DAsync(out->second_cost, out->second_cost_pitch, o.second_cost, o.second_cost_pitch, (size_t)W * 4, H, cudaMemcpyDeviceToHost, stream));
+        if (out->plane_index) FSW_CUDA(cudaMemcpy2DAsync(out->plane_index, out->plane_index_pitch, o.plane_index, o.plane_index_pitch, (size_t)W * 2, H, cudaMemcpyDeviceToHost, stream));
+        if (out->valid_reason) FSW_CUDA(cudaMemcpy2DAsync(out->valid_reason, out->valid_reason_pitch, o.valid_reason, o.valid_reason_pitch, (size_t)W, H, cudaMemcpyDeviceToHost, stream));
+    }
     FSW_CUDA(cudaStreamSynchronize(stream));
     return FSW_OK;
 }
@@ -700,7 +877,15 @@ int32_t fsw_compute_depth_host(fsw_context* ctx, const fsw_planeset* planes, con
                                const fsw_image* images, const uint8_t* mask, size_t mask_pitch,
                                const fsw_depth_out* out, void* cuda_stream) {
     fsw_rect none = {0, 0, 0, 0};
-    return run_host(ctx, false, planes, nullptr, params, nullptr, none, images, mask, mask_pitch, out, cuda_stream);
+    const uint8_t* masks[1] = {mask};
+    return run_host(ctx, false, planes, nullptr, params, nullptr, none, 1, images, mask ? masks : nullptr, mask_pitch, out, cuda_stream);
+}
+
+int32_t fsw_compute_depth_batch_host(fsw_context* ctx, const fsw_planeset* planes, const fsw_sweep_params* params,
+                                     int32_t n_sets, const fsw_image* images, const uint8_t* const* masks,
+                                     size_t mask_pitch, const fsw_depth_out* outs, void* cuda_stream) {
+    fsw_rect none = {0, 0, 0, 0};
+    return run_host(ctx, false, planes, nullptr, params, nullptr, none, n_sets, images, masks, mask_pitch, outs, cuda_stream);
 }
 
 int32_t fsw_compute_depth_multires_host(fsw_context* ctx, const fsw_planeset* planes_low,
@@ -708,7 +893,8 @@ int32_t fsw_compute_depth_multires_host(fsw_context* ctx, const fsw_planeset* pl
                                         const fsw_sweep_params* params_crop, fsw_rect crop, const fsw_image* images,
                                         const uint8_t* mask, size_t mask_pitch, const fsw_depth_out* out,
                                         void* cuda_stream) {
-    return run_host(ctx, true, planes_low, planes_crop, params_low, params_crop, crop, images, mask, mask_pitch, out, cuda_stream);
+    const uint8_t* masks[1] = {mask};
+    return run_host(ctx, true, planes_low, planes_crop, params_low, params_crop, crop, 1, images, mask ? masks : nullptr, mask_pitch, out, cuda_stream);
 }
 
 int32_t fsw_context_set_timing(fsw_context* ctx, int32_t on) {
@@ -729,7 +915,7 @@ int32_t fsw_get_last_counters(fsw_context* ctx, fsw_counters* out) {
     FSW_CUDA(g.enter(ctx->device));
     FSW_CUDA(cudaStreamSynchronize(ctx->last_stream));
     unsigned long long h[4] = {0, 0, 0, 0};
-    FSW_CUDA(cudaMemcpy(h, ctx->counters.p, sizeof(h), cudaMemcpyDeviceToHost));
+    FSW_CUDA(cudaMemcpy(h, ctx->counters(), sizeof(h), cudaMemcpyDeviceToHost));
     out->n_eval = (int64_t)h[0];
     out->n_raw_valid = (int64_t)h[1];
     out->n_valid = (int64_t)h[2];

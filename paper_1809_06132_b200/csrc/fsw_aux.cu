@@ -1,6 +1,6 @@
 /*
  * fsw_aux.cu -- the small kernels around the sweep:
- *   - footprint packing of 8-bit view images (so that one 32-bit load fetches the whole bilinear footprint, S4),
+ *   - footprint packing of the view images (one 128-bit load then fetches a whole bilinear footprint, S4),
  *   - the 2x2 box downsample of the two-scale strategy (PAPER.md:88-90, S10(a)),
  *   - an FFMA-chain kernel that measures the FP32 throughput used as the "alu" roofline denominator.
  */
@@ -8,43 +8,40 @@
 
 namespace {
 
-/* word(x,y) = I(x,y) | I(x+1,y)<<8 | I(x,y+1)<<16 | I(x+1,y+1)<<24, indices clamped at the right / bottom border
- * (a valid bilinear footprint never starts in the last column / row, so the clamped entries are never read). */
+__device__ __forceinline__ float load_px(const void* base, int64_t pitch, int dtype, int x, int y) {
+    const char* row = reinterpret_cast<const char*>(base) + (int64_t)y * pitch;
+    return dtype == FSW_U8 ? (float)__ldg(reinterpret_cast<const uint8_t*>(row) + x)
+                           : __ldg(reinterpret_cast<const float*>(row) + x);
+}
+
+/* foot(x,y) = (I(x,y), I(x+1,y) - I(x,y), I(x,y+1), I(x+1,y+1) - I(x,y+1)), indices clamped at the right / bottom
+ * border (a valid bilinear footprint never starts in the last column / row, so the clamped entries are never used).
+ * Two outputs per thread; a warp writes 1 KB of consecutive footprints. */
 __global__ void __launch_bounds__(256) pack_footprints_kernel(const __grid_constant__ FswPackArgs a) {
-    const int cam = blockIdx.z;
-    if (a.counters_to_zero != nullptr && cam == 0 && blockIdx.x == 0 && blockIdx.y == 0 && threadIdx.x < 4)
-        a.counters_to_zero[threadIdx.x] = 0ull;
-    const int W = a.W[cam], H = a.H[cam];
-    const int x4 = (blockIdx.x * blockDim.x + threadIdx.x) * 4; /* four outputs per thread */
+    const int img = blockIdx.z;
+    if (a.words_to_zero != nullptr && img == 0 && blockIdx.x == 0 && blockIdx.y == 0 && (int)threadIdx.x < a.n_words_to_zero)
+        a.words_to_zero[threadIdx.x] = 0u;
+    const int W = a.W, H = a.H;
+    const int x2 = (blockIdx.x * blockDim.x + threadIdx.x) * 2;
     const int y = blockIdx.y;
-    if (y >= H || x4 >= W) return;
-    const uint8_t* r0 = a.src[cam] + (int64_t)y * a.src_pitch[cam];
-    const uint8_t* r1 = a.src[cam] + (int64_t)min(y + 1, H - 1) * a.src_pitch[cam];
-    uint32_t t[5], b[5];
+    if (y >= H || x2 >= W) return;
+    const int y1 = min(y + 1, H - 1);
+    const int dt = a.dtype[img];
+    float t[3], b[3];
 #pragma unroll
-    for (int i = 0; i < 5; ++i) {
-        int x = min(x4 + i, W - 1);
-        t[i] = __ldg(r0 + x);
-        b[i] = __ldg(r1 + x);
+    for (int i = 0; i < 3; ++i) {
+        int x = min(x2 + i, W - 1);
+        t[i] = load_px(a.src[img], a.src_pitch[img], dt, x, y);
+        b[i] = load_px(a.src[img], a.src_pitch[img], dt, x, y1);
     }
-    uint32_t* dst = a.dst[cam] + (int64_t)y * W + x4;
-    uint32_t o[4];
-#pragma unroll
-    for (int i = 0; i < 4; ++i) o[i] = t[i] | (t[i + 1] << 8) | (b[i] << 16) | (b[i + 1] << 24);
-    if (x4 + 3 < W && (W & 3) == 0) {
-        *reinterpret_cast<uint4*>(dst) = make_uint4(o[0], o[1], o[2], o[3]);
-    } else {
-#pragma unroll
-        for (int i = 0; i < 4; ++i)
-            if (x4 + i < W) dst[i] = o[i];
-    }
+    float4* dst = a.dst[img] + (int64_t)y * W + x2;
+    dst[0] = make_float4(t[0], t[1] - t[0], b[0], b[1] - b[0]);
+    if (x2 + 1 < W) dst[1] = make_float4(t[1], t[2] - t[1], b[1], b[2] - b[1]);
 }
 
 /* out(x,y) = 0.25 * (I(2x,2y) + I(2x+1,2y) + I(2x,2y+1) + I(2x+1,2y+1)) as float32 */
 __global__ void __launch_bounds__(256) downsample_kernel(const __grid_constant__ FswDownArgs a) {
     const int cam = blockIdx.z;
-    if (a.counters_to_zero != nullptr && cam == 0 && blockIdx.x == 0 && blockIdx.y == 0 && threadIdx.x < 4)
-        a.counters_to_zero[threadIdx.x] = 0ull;
     const int W2 = a.W[cam] / 2, H2 = a.H[cam] / 2;
     const int x = blockIdx.x * blockDim.x + threadIdx.x;
     const int y = blockIdx.y;
@@ -81,12 +78,7 @@ __global__ void __launch_bounds__(256) ffma_peak_kernel(float* sink, int iters) 
 }  // namespace
 
 cudaError_t fsw_launch_pack_footprints(const FswPackArgs& args, cudaStream_t stream) {
-    int maxW = 0, maxH = 0;
-    for (int i = 0; i < args.n; ++i) {
-        maxW = args.W[i] > maxW ? args.W[i] : maxW;
-        maxH = args.H[i] > maxH ? args.H[i] : maxH;
-    }
-    dim3 grid((maxW + 4 * 256 - 1) / (4 * 256), maxH, args.n);
+    dim3 grid((args.W + 2 * 256 - 1) / (2 * 256), args.H, args.n);
     pack_footprints_kernel<<<grid, 256, 0, stream>>>(args);
     return cudaGetLastError();
 }

@@ -22,14 +22,17 @@
 #define FSW_DIST_K1 1   /* k1 only */
 #define FSW_DIST_FULL 2 /* k1,k2,p1,p2 */
 
-/* how a view image is stored on the device */
-#define FSW_PIX_FOOT_U8 0 /* footprint-packed: word(x,y) = I(x,y) | I(x+1,y)<<8 | I(x,y+1)<<16 | I(x+1,y+1)<<24 */
-#define FSW_PIX_F32 1     /* plain float32, pitch in elements */
+/* Footprint image of a matching view (S4): one float4 per pixel (x,y),
+ *   .x = I(x,y), .y = I(x+1,y) - I(x,y), .z = I(x,y+1), .w = I(x+1,y+1) - I(x,y+1)
+ * so that one 128-bit load fetches everything a bilinear sample needs:
+ *   top = .x + au*.y, bot = .z + au*.w, b = top + av*(bot - top).
+ * Built per frame set by pack_footprints_kernel (fsw_aux.cu) from 8-bit or float images; dense, pitch = W. */
 
 struct FswDevCam {
     float fx, fy, cx, cy, xi;
     float k1, k2, p1, p2;
-    float cos_fov; /* cos(fov_max/2) */
+    float cos_fov;     /* cos(fov_max/2) */
+    float cos_fov_xi;  /* cos(fov_max/2) + xi: the FOV test on cos(theta) + xi */
     int32_t W, H;
     int32_t dist_mode;
 };
@@ -39,9 +42,6 @@ struct FswDevView {
     float R[9]; /* reference -> view: X_v = R X_ref + T */
     float T[3];
     int32_t ident_R;  /* 1 if R is exactly the identity */
-    int32_t pix_mode; /* FSW_PIX_* */
-    const void* img;
-    int64_t pitch_elems; /* row pitch in elements (uint32 words or floats) */
 };
 
 struct FswDevFamily {
@@ -51,13 +51,34 @@ struct FswDevFamily {
     float s0, ds; /* spacing variable of plane j in the family: s0 + j*ds */
 };
 
-struct FswSweepArgs {
-    /* S1: reference camera and image */
-    FswDevCam ref;
+/* the buffers of one synchronized frame set */
+struct FswSetPtrs {
+    /* S1: reference image */
     const void* ref_img;
     int64_t ref_pitch_bytes;
     int32_t ref_dtype; /* FSW_U8 / FSW_F32 */
-    /* S3/S4: matching views, fixed order */
+    int32_t pad_;
+    /* S4: footprint images of the matching views, fixed view order, pitch = view width */
+    const float4* foot[FSW_MAX_VIEWS];
+    float* debug_cost; /* [P][H][W] or null */
+    /* S10 merge input (crop pass of the multi-resolution call): half-resolution raw maps, or null */
+    const float* lo_depth;
+    const float* lo_c1;
+    const float* lo_c2;
+    const int16_t* lo_k;
+    /* S11 */
+    const uint8_t* mask;
+    int64_t mask_pitch;
+    /* S12 outputs (device) */
+    float* out_depth;   int64_t out_depth_pitch;
+    float* out_c1;      int64_t out_c1_pitch;
+    float* out_c2;      int64_t out_c2_pitch;
+    int16_t* out_k;     int64_t out_k_pitch;
+    uint8_t* out_reason; int64_t out_reason_pitch;
+};
+
+struct FswSweepArgs {
+    FswDevCam ref;
     int32_t n_views;
     FswDevView views[FSW_MAX_VIEWS];
     /* S2: planes */
@@ -69,41 +90,42 @@ struct FswSweepArgs {
     int32_t roi_x0, roi_y0, roi_x1, roi_y1; /* clipped to the image, half-open */
     int32_t subpixel, filters, depth_kind, horizon_row;
     float alpha_upper, alpha_lower, beta;
-    float floor2;        /* (var_floor * N^2)^2, the floor applied to (N^2 var_a)(N^2 var_b) */
+    float floor2;        /* (var_floor * N)^2, the floor applied to (N var_a)(N var_b) */
     float inv_range_max; /* 1/range_max */
-    float* debug_cost;   /* [P][H][W] or null */
-    /* S10 merge input (crop pass of the multi-resolution call): half-resolution raw maps, or null */
-    const float* lo_depth;
-    const float* lo_c1;
-    const float* lo_c2;
-    const int16_t* lo_k;
+    float ref_rd2_max;   /* squared distorted normalised radius beyond which no reference pixel is inside the FOV
+                            (+inf when the bound does not apply): tiles entirely beyond it skip S1 */
     int32_t lo_W, lo_H;
     int32_t index_flag; /* OR-ed into the plane index this pass writes (FSW_INDEX_FROM_CROP or 0) */
-    /* S11 */
-    const uint8_t* mask;
-    int64_t mask_pitch;
-    /* S12 outputs (device) */
-    float* out_depth;   int64_t out_depth_pitch;
-    float* out_c1;      int64_t out_c1_pitch;
-    float* out_c2;      int64_t out_c2_pitch;
-    int16_t* out_k;     int64_t out_k_pitch;
-    uint8_t* out_reason; int64_t out_reason_pitch;
+    /* frame sets: set0 inline for the single-set calls, `sets` (device array) for batches */
+    int32_t n_sets;
+    FswSetPtrs set0;
+    const FswSetPtrs* sets;
+    /* work queue: items = n_sets * n_tiles, item i -> set i % n_sets, tile tile_order[i / n_sets] */
+    const int32_t* tile_order; /* device, n_tiles entries: tile index ty * n_tiles_x + tx, heaviest first */
+    int32_t n_tiles_x, n_tiles;
+    unsigned int* queue; /* zero before the launch; CTAs claim items beyond gridDim.x from it */
     /* counters: [0] n_eval, [1] n_raw_valid, [2] n_valid ([1],[2] only if count_pixels) */
     unsigned long long* counters;
     int32_t count_pixels;
 };
 
-/* launchers implemented in the .cu files; all enqueue on `stream` and return the launch status */
-cudaError_t fsw_launch_sweep(const FswSweepArgs& args, int window, cudaStream_t stream);
-cudaError_t fsw_sweep_prepare(int window); /* sets the dynamic shared memory attribute of that instantiation */
+/* geometry of the sweep kernel's tiles; fsw_api.cu needs it for the tile order and the grid */
+struct FswSweepGeometry {
+    int32_t tile_w, tile_h, threads, ctas_per_sm;
+    size_t smem_bytes;
+};
 
+/* launchers implemented in the .cu files; all enqueue on `stream` and return the launch status */
+#define FSW_PACK_MAX 64 /* images per pack launch */
 struct FswPackArgs {
-    int32_t n;
-    const uint8_t* src[FSW_MAX_CAMERAS];
-    int64_t src_pitch[FSW_MAX_CAMERAS];
-    uint32_t* dst[FSW_MAX_CAMERAS];
-    int32_t W[FSW_MAX_CAMERAS], H[FSW_MAX_CAMERAS];
-    unsigned long long* counters_to_zero; /* nullable: the first thread clears 4 counters */
+    int32_t n; /* images to pack in this launch (views of one or several frame sets), all W x H */
+    int32_t W, H;
+    const void* src[FSW_PACK_MAX];
+    int64_t src_pitch[FSW_PACK_MAX]; /* bytes */
+    int32_t dtype[FSW_PACK_MAX];
+    float4* dst[FSW_PACK_MAX];       /* dense [H][W] footprints */
+    unsigned int* words_to_zero;     /* nullable: the first threads clear n_words_to_zero 32-bit words (queue, counters) */
+    int32_t n_words_to_zero;
 };
 cudaError_t fsw_launch_pack_footprints(const FswPackArgs& args, cudaStream_t stream);
 
@@ -114,7 +136,6 @@ struct FswDownArgs {
     int32_t dtype[FSW_MAX_CAMERAS];
     float* dst[FSW_MAX_CAMERAS]; /* [H/2][W/2] dense */
     int32_t W[FSW_MAX_CAMERAS], H[FSW_MAX_CAMERAS];
-    unsigned long long* counters_to_zero;
 };
 cudaError_t fsw_launch_downsample(const FswDownArgs& args, cudaStream_t stream);
 

@@ -11,7 +11,8 @@
 #define FSW_CAT2(a, b) a##b
 #define FSW_CAT(a, b) FSW_CAT2(a, b)
 
-cudaError_t FSW_CAT(fsw_launch_sweep_w, FSW_WIN)(const FswSweepArgs& args, int variant, cudaStream_t stream) {
-    return fsw::launch_sweep_win<FSW_WIN>(args, variant, stream);
+cudaError_t FSW_CAT(fsw_launch_sweep_w, FSW_WIN)(const FswSweepArgs& args, int variant, int grid, cudaStream_t stream) {
+    return fsw::launch_sweep_win<FSW_WIN>(args, variant, grid, stream);
 }
 cudaError_t FSW_CAT(fsw_prepare_sweep_w, FSW_WIN)() { return fsw::prepare_sweep_win<FSW_WIN>(); }
+FswSweepGeometry FSW_CAT(fsw_geometry_sweep_w, FSW_WIN)(int n_views) { return fsw::geometry_win<FSW_WIN>(n_views); }

@@ -67,7 +67,7 @@ def test_config4_multires_merge_and_mask():
     k = test["plane_index"].astype(np.int32)
     assert not ((k[outside] >= 0) & ((k[outside] >> 14) & 1).astype(bool)).any()
     assert (test["depth"][mask != 0] == 0).all() and (test["valid_reason"][mask != 0] != 0).all()
-    assert counters["n_launches"] == 4  # downsample, low sweep, footprint pack, crop sweep
+    assert counters["n_launches"] == 5  # downsample, footprint pack + low sweep, footprint pack + crop sweep
 
 
 @pytest.mark.parametrize("frame", [0, 31])
@@ -200,3 +200,45 @@ def test_multires_host_call_small():
         ref, test, stats, _ = run_multires(cfg, images, mask, host=host)
         assert_gates(stats)
         assert (ref["kbest"] >> 14 == 1).any() and ((ref["kbest"] >= 0) & (ref["kbest"] >> 14 == 0)).any()
+
+
+def test_batch_equals_single_calls():
+    """fsw_compute_depth_batch: n frame sets in one sweep launch give exactly the maps of n separate calls
+    (device and host variants; masks may be missing for some sets), and the counters are the totals."""
+    import torch
+    import paper_1809_06132_b200 as fsw
+    cfg = _small_rig(W=150, H=77, n_views=2, fov=170.0)
+    _, _, ctx = gpu_objects(cfg)
+    planes = fsw.PlaneSet(cfg["families"])
+    p = dict(cfg["params"], filters=3, alpha_upper=0.3, alpha_lower=0.3, beta=1.1, horizon_row=40)
+    sets, masks = [], []
+    for s in range(5):
+        c = dict(cfg, scene=synth.scene_plane(2.0 + 0.7 * s, (0.5, 2.0), seed=20 + s))
+        sets.append(synth.render_frame(c, 0))
+        masks.append(synth.make_mask(150, 77, 30 + s, n_rects=2) if s % 2 == 0 else None)
+    singles, n_eval = [], 0
+    for s in range(5):
+        dev = [torch.from_numpy(im).cuda() for im in sets[s]]
+        dm = None if masks[s] is None else torch.from_numpy(masks[s]).cuda()
+        singles.append(oracle.compare.to_numpy(ctx.compute_depth(planes, p, dev, dm)))
+        n_eval += ctx.last_counters()["n_eval"]
+    dev_sets = [[torch.from_numpy(im).cuda() for im in st] for st in sets]
+    dev_masks = [None if m is None else torch.from_numpy(m).cuda() for m in masks]
+    outs = ctx.compute_depth_batch(planes, p, dev_sets, dev_masks)
+    torch.cuda.synchronize()
+    c = ctx.last_counters()
+    assert c["n_eval"] == n_eval and c["n_launches"] == 2
+    houts = ctx.compute_depth_batch(planes, p, sets, masks, host=True)
+    for s in range(5):
+        a, b = oracle.compare.to_numpy(outs[s]), oracle.compare.to_numpy(houts[s])
+        for key in ("depth", "best_cost", "second_cost", "plane_index", "valid_reason"):
+            assert np.array_equal(singles[s][key], a[key], equal_nan=True), (s, key)
+            assert np.array_equal(singles[s][key], b[key], equal_nan=True), (s, key)
+        if masks[s] is not None:
+            assert (a["depth"][masks[s] != 0] == 0).all()
+    # one set against the oracle, so that the batch path is pinned to more than itself
+    ref = oracle.compute_depth(cfg["cams"], cfg["ref_index"], cfg["families"], p, sets[3], masks[3], keep_cost=True)
+    st = oracle.compare.compare_maps(ref, oracle.compare.to_numpy(outs[3]), ref["cost"])
+    assert st["index_match_frac"] >= 0.999 and st["max_dc1"] <= 1e-4 and st["valid_mismatch_nonfragile"] == 0, st
+    with pytest.raises(fsw.FswError):
+        ctx.compute_depth_batch(planes, p, [], None)
