@@ -37,6 +37,8 @@ def parse_args():
     ap.add_argument("--steps", type=int, default=128)
     ap.add_argument("--warmup", type=int, default=8)
     ap.add_argument("--workload", default="C5", choices=["C5", "C3"])
+    ap.add_argument("--batch", type=int, default=8,
+                    help="frame sets per sweep launch (fsw_compute_depth_batch); 1 = one launch per frame set")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--cpu-baseline-seconds", type=float, default=12.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -211,9 +213,30 @@ def run_ours(args, rank, local_rank, world):
                  plane_index=torch.empty((H, W), dtype=torch.int16, device=dev),
                  valid_reason=torch.empty((H, W), dtype=torch.uint8, device=dev)) for _ in range(N_STAGED)]
 
+    B = max(1, min(args.batch, N_STAGED))
+
     def step(i):
         f = i % N_STAGED
         ctx.compute_depth(planes, cfg["params"], dev_frames[f], dev_masks[f], out=outs[f])
+
+    def run_steps(first, n, host=False):
+        """steps first .. first+n-1, B consecutive frame sets per launch (the stream is processed in order)"""
+        i = first
+        while i < first + n:
+            nb = min(B, first + n - i)
+            fs = [(i + j) % N_STAGED for j in range(nb)]
+            if host:
+                if nb == 1:
+                    ctx.compute_depth(planes, cfg["params"], pin_frames[fs[0]], pin_masks[fs[0]], host=True, out=pin_outs[0])
+                else:
+                    ctx.compute_depth_batch(planes, cfg["params"], [pin_frames[f] for f in fs],
+                                            [pin_masks[f] for f in fs], want=("depth",), host=True, outs=pin_outs[:nb])
+            elif nb == 1:
+                step(i)
+            else:
+                ctx.compute_depth_batch(planes, cfg["params"], [dev_frames[f] for f in fs], [dev_masks[f] for f in fs],
+                                        outs=[outs[f] for f in fs])
+            i += nb
 
     def barrier():
         if dist is not None:
@@ -221,8 +244,7 @@ def run_ours(args, rank, local_rank, world):
         torch.cuda.synchronize()
 
     # ---- device-resident timing ------------------------------------------------------------------------------------
-    for i in range(args.warmup):
-        step(i)
+    run_steps(0, args.warmup)
     torch.cuda.synchronize()
     n_eval_step = []
     launches = 0
@@ -237,49 +259,52 @@ def run_ours(args, rank, local_rank, world):
     barrier()
     sampler.start()
     ev0.record(stream)
-    for i in range(args.steps):
-        step(i)
+    run_steps(0, args.steps)
     ev1.record(stream)
     torch.cuda.synchronize()
     sampler.stop_flag = True
     barrier()
     ms_total = ev0.elapsed_time(ev1)
-    launches = launches_per_step * args.steps
+    n_calls = (args.steps + B - 1) // B
+    launches = launches_per_step * n_calls
     evals_total = float(sum(n_eval_step[i % len(n_eval_step)] for i in range(args.steps)))
 
     # ---- the sweep kernel alone: CUDA events around its launches on the same stream (fsw_context_set_timing) ------
     ctx.set_timing(True)
-    sweep_ms = []
-    for i in range(min(args.steps, 2 * N_STAGED)):
-        step(i)
+    sweep_ms, sweep_evals = [], []
+    for i in range(0, min(args.steps, 2 * N_STAGED) // B * B, B):
+        run_steps(i, B)
         sweep_ms.append(ctx.last_counters()["sweep_ms"])
+        sweep_evals.append(sum(n_eval_step[(i + j) % len(n_eval_step)] for j in range(B)))
     ctx.set_timing(False)
     sweep_ms_avg = float(np.mean(sweep_ms))
-    evals_per_launch = float(np.mean([n_eval_step[i % len(n_eval_step)] for i in range(len(sweep_ms))]))
+    evals_per_launch = float(np.mean(sweep_evals))
+    # latency of a single frame set (one launch per frame set), for context
+    torch.cuda.synchronize()
+    ev0.record(stream)
+    for i in range(8):
+        step(i)
+    ev1.record(stream)
+    torch.cuda.synchronize()
+    ms_single = ev0.elapsed_time(ev1) / 8
 
     # ---- end to end: host buffers through fsw_compute_depth_host ---------------------------------------------------
     pin_frames = [[torch.from_numpy(im).pin_memory() for im in fr] for fr in host_frames]
     pin_masks = [torch.from_numpy(m).pin_memory() for m in host_masks] or [None] * N_STAGED
-    pin_out = dict(depth=torch.empty((H, W), dtype=torch.float32).pin_memory())
+    pin_outs = [dict(depth=torch.empty((H, W), dtype=torch.float32).pin_memory()) for _ in range(B)]
     h2d = sum(int(t.numel() * t.element_size()) for t in pin_frames[0]) + (W * H if host_masks else 0)
     d2h = W * H * 4
 
-    def step_e2e(i):
-        f = i % N_STAGED
-        ctx.compute_depth(planes, cfg["params"], pin_frames[f], pin_masks[f], host=True, out=pin_out)
-
-    for i in range(3):
-        step_e2e(i)
+    run_steps(0, 3 * B, host=True)
     e2e_steps = args.steps
     barrier()
     ev0.record(stream)
-    for i in range(e2e_steps):
-        step_e2e(i)
+    run_steps(0, e2e_steps, host=True)
     ev1.record(stream)
     torch.cuda.synchronize()
     barrier()
     ms_e2e = ev0.elapsed_time(ev1)
-    launches += launches_per_step * e2e_steps
+    launches += launches_per_step * n_calls
 
     # ---- max over ranks ----------------------------------------------------------------------------------------------
     (ms_total, ms_e2e), (evals_all,) = shard.reduce_timing([ms_total, ms_e2e], [evals_total], dev)
@@ -297,6 +322,7 @@ def run_ours(args, rank, local_rank, world):
                        "n_eval_per_step": evals_total / args.steps, "n_nominal_per_step": W * H * planes.n_planes * (rig.n_cams - 1),
                        "l2": "inputs and outputs rotate over %d distinct frame sets (%.0f MB per pass) > 126 MB L2" % (
                            N_STAGED, N_STAGED * (3 * W * H + W * H + W * H * 15 + 2 * W * H * 4) / 1e6),
+                       "frame_sets_per_launch": B, "ms_single_frame_set_launch": ms_single,
                        "parallelism": "frame sets sharded over %d GPU(s), no collective" % world},
             "depth_maps_per_s": world * args.steps / (ms_total * 1e-3) if dist is None else None,
             "clocks": sampler.summary(),

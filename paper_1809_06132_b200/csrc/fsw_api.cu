@@ -192,6 +192,7 @@ FswDevCam dev_cam(const fsw_camera& c, bool half) {
     d.cos_fov = (float)std::cos(0.5 * c.fov_max_deg * M_PI / 180.0);
     d.cos_fov_xi = (float)(std::cos(0.5 * c.fov_max_deg * M_PI / 180.0) + c.xi);
     d.W = W; d.H = H;
+    d.Wm1 = W - 1; d.Hm1 = H - 1;
     if (c.k1 == 0.0 && c.k2 == 0.0 && c.p1 == 0.0 && c.p2 == 0.0) d.dist_mode = FSW_DIST_NONE;
     else if (c.k2 == 0.0 && c.p1 == 0.0 && c.p2 == 0.0) d.dist_mode = FSW_DIST_K1;
     else d.dist_mode = FSW_DIST_FULL;
@@ -304,6 +305,7 @@ int32_t fill_args(FswSweepArgs& a, const fsw_rig& rig, const fsw_planeset& ps, c
     a.floor2 = (float)(fl * fl);
     if (!(a.floor2 > 0.f)) a.floor2 = 1e-30f; /* keeps the reciprocal square root finite on flat windows */
     a.inv_range_max = 1.f / p.range_max;
+    for (int c = 0; c < FSW_MAX_CAMERAS; ++c) a.inv_count[c] = c > 0 ? 1.f / (float)c : 0.f;
     a.n_sets = 1;
     return FSW_OK;
 }
@@ -337,14 +339,14 @@ FswSweepGeometry window_geometry(int w, int n_views) {
 }
 
 /* picks the kernel variant the views allow (see fsw_sweep.cuh) */
-int pick_variant(const FswSweepArgs& a) {
+int pick_variant(const FswSweepArgs& a, int foot_f16) {
     bool fast = true;
     for (int v = 0; v < a.n_views; ++v) {
         fast = fast && a.views[v].ident_R;
         fast = fast && a.views[v].cam.dist_mode != FSW_DIST_FULL;
         fast = fast && (a.views[v].cam.cos_fov_xi >= 1e-3f); /* lets the kernel drop the denominator test */
     }
-    return fast ? 1 : 0;
+    return (fast ? 1 : 0) | (foot_f16 ? 2 : 0);
 }
 
 /* Scheduling order of the tiles (S0): nearest to the principal point first, lower image half before the upper
@@ -399,7 +401,7 @@ int32_t launch_sweep(fsw_context* ctx, FswSweepArgs& a, int w, cudaStream_t s) {
     const long long items = (long long)a.n_tiles * a.n_sets;
     const long long slots = (long long)ctx->n_sm * g.ctas_per_sm;
     const int grid = (int)(items < slots ? items : slots);
-    const int var = pick_variant(a);
+    const int var = pick_variant(a, a.foot_f16);
     cudaError_t e = cudaErrorInvalidValue;
     switch (w) {
         case 3: e = fsw_launch_sweep_w3(a, var, grid, s); break;
@@ -419,8 +421,14 @@ int32_t launch_sweep(fsw_context* ctx, FswSweepArgs& a, int w, cudaStream_t s) {
  * context scratch and records the pointers in sets[]; the first pack launch also clears the work queue (and the
  * counters if asked).  half = the images are the context's half-resolution float images. */
 int32_t stage_views(fsw_context* ctx, const fsw_image* images, int n_sets, bool half, FswSetPtrs* sets,
-                    cudaStream_t stream, bool zero_counters) {
+                    cudaStream_t stream, bool zero_counters, int32_t* foot_f16) {
     const fsw_rig& rig = ctx->rig;
+    /* 8-byte bfloat16 footprints when every view of the call is an 8-bit image (exact), 16-byte float ones otherwise */
+    int f16 = half ? 0 : 1;
+    for (int s = 0; s < n_sets && f16; ++s)
+        for (int c = 0; c < rig.n_cams; ++c)
+            if (c != rig.ref_index && images[(size_t)s * rig.n_cams + c].dtype != FSW_U8) f16 = 0;
+    *foot_f16 = f16;
     if (!half && ctx->foot.size() < (size_t)n_sets * FSW_MAX_CAMERAS) ctx->foot.resize((size_t)n_sets * FSW_MAX_CAMERAS);
     bool first = true;
     /* one launch per camera size (all views of a rig usually share one) and per FSW_PACK_MAX images */
@@ -431,7 +439,7 @@ int32_t stage_views(fsw_context* ctx, const fsw_image* images, int n_sets, bool 
         const int H = half ? rig.cams[c0].height / 2 : rig.cams[c0].height;
         FswPackArgs pk;
         std::memset(&pk, 0, sizeof(pk));
-        pk.W = W; pk.H = H;
+        pk.W = W; pk.H = H; pk.f16 = f16;
         auto flush = [&]() -> int32_t {
             if (pk.n == 0) return FSW_OK;
             if (first) {
@@ -463,8 +471,8 @@ int32_t stage_views(fsw_context* ctx, const fsw_image* images, int n_sets, bool 
                     const fsw_image& im = images[(size_t)s * rig.n_cams + c];
                     pk.src[pk.n] = im.data; pk.src_pitch[pk.n] = (int64_t)im.pitch_bytes; pk.dtype[pk.n] = im.dtype;
                 }
-                pk.dst[pk.n] = (float4*)fb.p;
-                sets[s].foot[vi] = (const float4*)fb.p;
+                pk.dst[pk.n] = fb.p;
+                sets[s].foot[vi] = fb.p;
                 pk.n++;
                 if (pk.n == FSW_PACK_MAX) {
                     int32_t rc = flush();
@@ -690,7 +698,7 @@ static int32_t run_sets(fsw_context* ctx, const fsw_planeset* planes, const fsw_
         sets[s].debug_cost = params->debug_cost_volume;
         set_outputs(sets[s], &outs[s], masks ? masks[s] : nullptr, mask_pitch);
     }
-    if ((rc = stage_views(ctx, images, n_sets, false, sets.data(), stream, true)) != FSW_OK) return rc;
+    if ((rc = stage_views(ctx, images, n_sets, false, sets.data(), stream, true, &a.foot_f16)) != FSW_OK) return rc;
     a.n_sets = n_sets;
     a.set0 = sets[0];
     if (n_sets > 1) {
@@ -774,7 +782,7 @@ int32_t fsw_compute_depth_multires(fsw_context* ctx, const fsw_planeset* planes_
     lo.out_c1 = (float*)ctx->lo_c1.p; lo.out_c1_pitch = (int64_t)LW * 4;
     lo.out_c2 = (float*)ctx->lo_c2.p; lo.out_c2_pitch = (int64_t)LW * 4;
     lo.out_k = (int16_t*)ctx->lo_k.p; lo.out_k_pitch = (int64_t)LW * 2;
-    if ((rc = stage_views(ctx, nullptr, 1, true, &lo, stream, true)) != FSW_OK) return rc;
+    if ((rc = stage_views(ctx, nullptr, 1, true, &lo, stream, true, &a.foot_f16)) != FSW_OK) return rc;
     a.set0 = lo;
     a.count_pixels = 0;
     ctx->n_timed = 0;
@@ -793,7 +801,7 @@ int32_t fsw_compute_depth_multires(fsw_context* ctx, const fsw_planeset* planes_
     set_outputs(hi, out, mask, mask_pitch);
     hi.lo_depth = (const float*)ctx->lo_depth.p; hi.lo_c1 = (const float*)ctx->lo_c1.p; hi.lo_c2 = (const float*)ctx->lo_c2.p;
     hi.lo_k = (const int16_t*)ctx->lo_k.p;
-    if ((rc = stage_views(ctx, images, 1, false, &hi, stream, false)) != FSW_OK) return rc;
+    if ((rc = stage_views(ctx, images, 1, false, &hi, stream, false, &a.foot_f16)) != FSW_OK) return rc;
     a.set0 = hi;
     a.lo_W = LW; a.lo_H = LH;
     a.index_flag = FSW_INDEX_FROM_CROP;

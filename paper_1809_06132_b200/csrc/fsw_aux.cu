@@ -1,6 +1,6 @@
 /*
  * fsw_aux.cu -- the small kernels around the sweep:
- *   - footprint packing of the view images (one 128-bit load then fetches a whole bilinear footprint, S4),
+ *   - footprint packing of the view images (one 64- or 128-bit load then fetches a whole bilinear footprint, S4),
  *   - the 2x2 box downsample of the two-scale strategy (PAPER.md:88-90, S10(a)),
  *   - an FFMA-chain kernel that measures the FP32 throughput used as the "alu" roofline denominator.
  */
@@ -12,6 +12,11 @@ __device__ __forceinline__ float load_px(const void* base, int64_t pitch, int dt
     const char* row = reinterpret_cast<const char*>(base) + (int64_t)y * pitch;
     return dtype == FSW_U8 ? (float)__ldg(reinterpret_cast<const uint8_t*>(row) + x)
                            : __ldg(reinterpret_cast<const float*>(row) + x);
+}
+
+/* (value, difference) as two bfloat16 in one word: value in the low half */
+__device__ __forceinline__ unsigned pack_bf16(float v, float d) {
+    return (__float_as_uint(v) >> 16) | (__float_as_uint(d) & 0xffff0000u);
 }
 
 /* foot(x,y) = (I(x,y), I(x+1,y) - I(x,y), I(x,y+1), I(x+1,y+1) - I(x,y+1)), indices clamped at the right / bottom
@@ -34,9 +39,20 @@ __global__ void __launch_bounds__(256) pack_footprints_kernel(const __grid_const
         t[i] = load_px(a.src[img], a.src_pitch[img], dt, x, y);
         b[i] = load_px(a.src[img], a.src_pitch[img], dt, x, y1);
     }
-    float4* dst = a.dst[img] + (int64_t)y * W + x2;
-    dst[0] = make_float4(t[0], t[1] - t[0], b[0], b[1] - b[0]);
-    if (x2 + 1 < W) dst[1] = make_float4(t[1], t[2] - t[1], b[1], b[2] - b[1]);
+    if (a.f16) { /* integers up to 256 are exact in bfloat16 = the upper half of the float */
+        uint2* dst = reinterpret_cast<uint2*>(a.dst[img]) + (int64_t)y * W + x2;
+        const uint2 f0 = make_uint2(pack_bf16(t[0], t[1] - t[0]), pack_bf16(b[0], b[1] - b[0]));
+        const uint2 f1 = make_uint2(pack_bf16(t[1], t[2] - t[1]), pack_bf16(b[1], b[2] - b[1]));
+        if (x2 + 1 < W && (W & 1) == 0) *reinterpret_cast<uint4*>(dst) = make_uint4(f0.x, f0.y, f1.x, f1.y);
+        else {
+            dst[0] = f0;
+            if (x2 + 1 < W) dst[1] = f1;
+        }
+    } else {
+        float4* dst = reinterpret_cast<float4*>(a.dst[img]) + (int64_t)y * W + x2;
+        dst[0] = make_float4(t[0], t[1] - t[0], b[0], b[1] - b[0]);
+        if (x2 + 1 < W) dst[1] = make_float4(t[1], t[2] - t[1], b[1], b[2] - b[1]);
+    }
 }
 
 /* out(x,y) = 0.25 * (I(2x,2y) + I(2x+1,2y) + I(2x,2y+1) + I(2x+1,2y+1)) as float32 */

@@ -22,10 +22,12 @@
 #define FSW_DIST_K1 1   /* k1 only */
 #define FSW_DIST_FULL 2 /* k1,k2,p1,p2 */
 
-/* Footprint image of a matching view (S4): one float4 per pixel (x,y),
+/* Footprint image of a matching view (S4): four numbers per pixel (x,y),
  *   .x = I(x,y), .y = I(x+1,y) - I(x,y), .z = I(x,y+1), .w = I(x+1,y+1) - I(x,y+1)
- * so that one 128-bit load fetches everything a bilinear sample needs:
+ * so that one load fetches everything a bilinear sample needs:
  *   top = .x + au*.y, bot = .z + au*.w, b = top + av*(bot - top).
+ * Stored as four floats (128-bit load), or -- when every view of the call is an 8-bit image -- as four bfloat16
+ * (64-bit load: integers up to 256 and their differences are exact in bfloat16; half the cache footprint).
  * Built per frame set by pack_footprints_kernel (fsw_aux.cu) from 8-bit or float images; dense, pitch = W. */
 
 struct FswDevCam {
@@ -34,6 +36,7 @@ struct FswDevCam {
     float cos_fov;     /* cos(fov_max/2) */
     float cos_fov_xi;  /* cos(fov_max/2) + xi: the FOV test on cos(theta) + xi */
     int32_t W, H;
+    int32_t Wm1, Hm1;  /* W - 1, H - 1: a bilinear footprint starts at 0 <= floor(u) < W - 1, 0 <= floor(v) < H - 1 */
     int32_t dist_mode;
 };
 
@@ -59,7 +62,7 @@ struct FswSetPtrs {
     int32_t ref_dtype; /* FSW_U8 / FSW_F32 */
     int32_t pad_;
     /* S4: footprint images of the matching views, fixed view order, pitch = view width */
-    const float4* foot[FSW_MAX_VIEWS];
+    const void* foot[FSW_MAX_VIEWS];
     float* debug_cost; /* [P][H][W] or null */
     /* S10 merge input (crop pass of the multi-resolution call): half-resolution raw maps, or null */
     const float* lo_depth;
@@ -92,9 +95,11 @@ struct FswSweepArgs {
     float alpha_upper, alpha_lower, beta;
     float floor2;        /* (var_floor * N)^2, the floor applied to (N var_a)(N var_b) */
     float inv_range_max; /* 1/range_max */
+    float inv_count[FSW_MAX_CAMERAS]; /* 1/c for c valid views (S6: mean over the valid views) */
     float ref_rd2_max;   /* squared distorted normalised radius beyond which no reference pixel is inside the FOV
                             (+inf when the bound does not apply): tiles entirely beyond it skip S1 */
     int32_t lo_W, lo_H;
+    int32_t foot_f16;   /* 1: the footprint images hold four bfloat16 per pixel, 0: four floats */
     int32_t index_flag; /* OR-ed into the plane index this pass writes (FSW_INDEX_FROM_CROP or 0) */
     /* frame sets: set0 inline for the single-set calls, `sets` (device array) for batches */
     int32_t n_sets;
@@ -123,7 +128,8 @@ struct FswPackArgs {
     const void* src[FSW_PACK_MAX];
     int64_t src_pitch[FSW_PACK_MAX]; /* bytes */
     int32_t dtype[FSW_PACK_MAX];
-    float4* dst[FSW_PACK_MAX];       /* dense [H][W] footprints */
+    void* dst[FSW_PACK_MAX];         /* dense [H][W] footprints */
+    int32_t f16;                     /* 1: four bfloat16 per footprint (8 bytes), 0: four floats (16 bytes) */
     unsigned int* words_to_zero;     /* nullable: the first threads clear n_words_to_zero 32-bit words (queue, counters) */
     int32_t n_words_to_zero;
 };

@@ -1,16 +1,16 @@
 /*
  * fsw_sweep.cuh -- the fused fisheye plane-sweep kernel (sm_100a), steps S1..S12 of SURVEY.md section 8(a).
  *
- * Persistent CTAs claim (frame set, tile) items from a queue, heaviest tiles first.  For one TX x TY tile of
- * reference pixels a CTA
+ * Persistent CTAs (one per SM, 16 warps) claim (frame set, tile) items from a queue, heaviest tiles first.  For one
+ * TX x TY tile of reference pixels a CTA
  *   S1  back-projects the tile plus a halo of w/2 pixels through the unified model (Eq. 1) into
  *       shared memory (no ray LUT ever touches HBM),
- *   and then, for every sweep plane k,
- *   S2-S4 maps every halo pixel through the plane into ALL matching views in one pass (ray-homography form
- *       X' ~ R r + (n.r / d_k) T; the incidence n.r and the range test are shared by the views), projects it with
- *       each view's fisheye model and samples the view bilinearly from its footprint image (one 128-bit load),
- *   S5  forms the windowed sums of b, b^2, ab with separable sliding box sums staged in shared memory and scores
- *       cost = (1 - ZNCC)/2,
+ *   and then, for every sweep plane k and every matching view,
+ *   S2-S4 maps every halo pixel through the plane into the view (ray-homography form X' ~ R r + (n.r / d_k) T),
+ *       projects it with the view's fisheye model and samples the view bilinearly from its footprint image (one
+ *       128-bit load),
+ *   S5  forms the windowed sums of b, b^2, ab with separable sliding box sums and scores cost = (1 - ZNCC)/2
+ *       (PAPER.md:76),
  *   S6  averages the cost over the views whose window is fully valid,
  *   S7  keeps best cost, non-adjacent second best and the neighbours of the best in registers --
  *       the cost volume is never written unless a debug buffer is given,
@@ -18,9 +18,14 @@
  *   S8-S12 refines the plane with a parabola, converts to depth, merges with the half-resolution pass if one is
  *       given, applies the cost / ratio filters and the mask and
  *       stores the maps with coalesced row writes.
- * Planes that no ray of the tile can reach within range_max are skipped without sampling.
  *
- * Two block-wide barriers per plane: sample -> [A] -> horizontal sums -> [B] -> vertical sums, ZNCC, WTA.
+ * Work split.  Warp w owns R consecutive halo rows of the tile for the whole tile: it samples them (S2-S4) into its
+ * private rows of the sample plane and immediately runs the horizontal box sums over them (a __syncwarp, no block
+ * barrier, in between); the reference-side operands a' of its horizontal work item stay in registers for the whole
+ * sweep.  After one block barrier every thread does the vertical sums, the ZNCC and the winner-take-all update of its
+ * own RPT output pixels; the second barrier of a (plane, view) pass sits right after the loads of the vertical pass,
+ * so its arithmetic overlaps the next pass of faster warps.  Row groups that no ray can reach (outside the image
+ * circle, above the horizon for ground-parallel planes, beyond range_max) are skipped per warp, whole planes per tile.
  *
  * Numerics: everything is FP32, no fast-math.  Intensities are centred on a per-tile constant before any sum
  * (ZNCC is invariant to offsets) so that Sum(b^2) - Sum(b)^2/N does not cancel catastrophically.
@@ -36,33 +41,38 @@ namespace fsw {
 
 constexpr int RUN = 8; /* outputs per work item of the horizontal pass */
 
-/* tile geometry: TX x TY outputs, NT threads; thread t owns column t % TX and RPT consecutive rows */
-template <int WIN, int TX_, int TY_, int NT_, int MINB_>
+/* tile geometry: 64 x TY outputs, 512 threads; thread t owns column t % 64 and RPT consecutive rows; warp w owns the
+ * R halo rows w*R .. w*R+R-1 in the sample / horizontal phase.  The sample planes have a row stride of SB = EW rounded
+ * up to a multiple of 4 and no other padding, so that lane l's i-th halo pixel of the warp's rows sits at the fixed
+ * offset l + 32 i from the warp's first row (the up to 3 extra columns of a row are sampled like halo pixels). */
+template <int WIN>
 struct Geo {
-    static constexpr int TX = TX_, TY = TY_, NT = NT_, MINB = MINB_;
+    static constexpr int TX = 64, NT = 512, MINB = 1;
     static constexpr int NW = NT / 32;
-    static constexpr int NG = NT / TX;       /* row groups */
-    static constexpr int RPT = TY / NG;      /* output rows per thread */
+    static constexpr int NG = NT / TX;                 /* row groups of the vertical pass */
+    static constexpr int R = WIN <= 9 ? 3 : 4;         /* halo rows per warp */
+    static constexpr int RPT = WIN <= 9 ? 5 : 6;       /* output rows per thread */
+    static constexpr int TY = NG * RPT;
     static constexpr int NRUN = TX / RUN;
     static constexpr int HW = WIN / 2;
-    static constexpr int EW = TX + 2 * HW;   /* tile + halo */
+    static constexpr int EW = TX + 2 * HW;             /* tile + halo */
     static constexpr int EH = TY + 2 * HW;
-    static constexpr int NE = EW * EH;       /* halo pixels = samples per plane and view */
-    static constexpr int NS = (NE + NT - 1) / NT; /* samples per thread */
-    static constexpr int NV = RUN + 2 * HW;        /* values one horizontal work item reads */
-    static constexpr int NV4 = (NV + 3) / 4;       /* ... as 128-bit loads */
-    /* row stride of the sample planes: covers the last run's 128-bit loads and is == 4 (mod 8) words so that
-     * 128-bit accesses of consecutive rows are bank-conflict free */
+    static constexpr int EHA = R * NW;                 /* allocated halo rows */
+    static constexpr int NV = RUN + 2 * HW;            /* values one horizontal work item reads */
+    static constexpr int NV4 = (NV + 3) / 4;           /* ... as 128-bit loads */
     static constexpr int SBMIN = ((NRUN - 1) * RUN + NV4 * 4) > EW ? ((NRUN - 1) * RUN + NV4 * 4) : EW;
-    static constexpr int SB = (SBMIN + 7) / 8 * 8 + 4 >= SBMIN + 8 ? (SBMIN + 7) / 8 * 8 - 4 : (SBMIN + 7) / 8 * 8 + 4;
-    static constexpr int HS = TX + 4;              /* row stride of the row-sum planes, == 4 (mod 8) */
-    static constexpr int PLANE = EH * SB;
-    static constexpr int HPLANE = EH * HS;
-    static constexpr int NHITEM = EH * NRUN;       /* work items of the horizontal pass (per view) */
-    static_assert(NT % TX == 0 && TY % NG == 0 && TX % 32 == 0 && TX % RUN == 0, "tile / thread mapping");
-    static_assert(SB >= SBMIN && SB % 8 == 4 && HS % 8 == 4, "bank-conflict-free strides");
-    static constexpr size_t smem(int vc) {
-        return sizeof(float4) * PLANE + sizeof(float) * ((size_t)PLANE * (1 + vc) + (size_t)4 * HPLANE * vc);
+    static constexpr int SB = (SBMIN + 3) / 4 * 4;     /* row stride of the sample planes */
+    static constexpr int NS = (R * SB + 31) / 32;      /* sample slots per lane */
+    static constexpr int NSFULL = (R * SB) / 32;       /* slots in which every lane has a pixel */
+    static constexpr int HS = TX + 4;                  /* row stride of the row-sum planes, == 4 (mod 8) */
+    static constexpr int PLANE = EHA * SB;
+    static constexpr int HPLANE = EHA * HS;
+    static constexpr bool A_IN_REGS = WIN <= 9;        /* keep the a' operands of the horizontal item in registers */
+    static_assert(EH <= EHA && TX % 32 == 0 && TX % RUN == 0 && NRUN == 8, "tile / thread mapping");
+    static_assert(SB >= SBMIN && SB % 4 == 0 && HS % 8 == 4, "aligned strides");
+    static_assert(R * NRUN <= 32, "one horizontal work item per lane");
+    static constexpr size_t smem() {
+        return sizeof(float4) * PLANE + sizeof(float) * ((size_t)2 * PLANE + (size_t)4 * HPLANE);
     }
 };
 
@@ -134,15 +144,16 @@ __device__ inline bool back_project(const FswDevCam& c, float u, float v, float&
     return rz >= c.cos_fov; /* theta <= fov/2 */
 }
 
-/* S3-S4 for one halo pixel and one view: bilinear sample of the view at the plane-induced position minus `centre`,
- * or NaN if the pixel / plane / view combination is invalid ("NONE" of SURVEY 8(b)).
+/* S3-S4 for one halo pixel and one view: bilinear sample of the view at the plane-induced position minus `centre`;
+ * `ok` is false (and the value NaN) if the pixel / plane / view combination is invalid ("NONE" of SURVEY 8(b)).
  * (rx,ry,rz) is the reference ray, s = (n.r)/d_k the inverse range along it (NaN if the ray misses the plane or the
- * intersection is beyond range_max: the NaN then fails the image-bounds test below, no separate flag is carried).
+ * intersection is beyond range_max: the NaN then fails the field-of-view test below, no separate flag is carried).
  * IDENT: the view's relative rotation is the identity.  FULLDIST: k2 / p1 / p2 may be non-zero.
- * CHECKDEN: cos(fov/2) + xi may be < 1e-3, so the projection denominator is tested on its own. */
-template <bool IDENT, bool FULLDIST, bool CHECKDEN>
+ * CHECKDEN: cos(fov/2) + xi may be < 1e-3, so the projection denominator is tested on its own.
+ * F16: the footprint images hold four bfloat16 per pixel (8-bit views) instead of four floats. */
+template <bool IDENT, bool FULLDIST, bool CHECKDEN, bool F16>
 __device__ __forceinline__ float warp_sample(float rx, float ry, float rz, float s, const FswDevView& k,
-                                             const float4* __restrict__ foot, float centre) {
+                                             const void* __restrict__ foot, float centre, bool& ok) {
     /* S2: X' ~ R r + s T */
     float X, Y, Z;
     if (IDENT) {
@@ -158,7 +169,7 @@ __device__ __forceinline__ float warp_sample(float rx, float ry, float rz, float
     float rho2 = fmaf(X, X, fmaf(Y, Y, Z * Z));
     float irho = rsqrt_approx(rho2);
     float t = fmaf(Z, irho, k.cam.xi);       /* cos(theta) + xi; NaN for rho2 == 0 */
-    bool ok = t >= k.cam.cos_fov_xi;         /* theta <= fov/2; false for NaN */
+    ok = t >= k.cam.cos_fov_xi;              /* theta <= fov/2; false for NaN */
     if (CHECKDEN) ok = ok && (t > FSW_EPS_DEN);
     float g = irho * rcp_approx(t);
     float mx = X * g, my = Y * g;
@@ -178,24 +189,29 @@ __device__ __forceinline__ float warp_sample(float rx, float ry, float rz, float
     /* floor without a float->int conversion: adding 1.5 * 2^23 with round-down leaves floor(u) in the low mantissa
      * bits (two's complement for negative values); anything with |u| >= 2^22, infinities and NaN fail the test */
     float tu = __fadd_rd(u, 12582912.f), tv = __fadd_rd(v, 12582912.f);
-    int ix = __float_as_int(tu) - 0x4B400000, iy = __float_as_int(tv) - 0x4B400000;
+    unsigned ix = (unsigned)__float_as_int(tu) - 0x4B400000u, iy = (unsigned)__float_as_int(tv) - 0x4B400000u;
     /* bilinear footprint inside the view image: 0 <= u < W-1, 0 <= v < H-1  <=>  0 <= floor(u) < W-1, ... */
-    ok = ok && ((unsigned)ix < (unsigned)(k.cam.W - 1)) && ((unsigned)iy < (unsigned)(k.cam.H - 1));
-    float b = CUDART_NAN_F;
-    if (ok) {
-        /* S4: one point fetch of the footprint + FP32 lerp (hardware texture filtering has 8-bit weights: too
-         * coarse for the 1e-4 cost tolerance) */
-        float au = u - (tu - 12582912.f);
-        float av = v - (tv - 12582912.f);
-        float4 f = __ldg(foot + (iy * k.cam.W + ix));
-        float top = fmaf(au, f.y, f.x);
-        float bot = fmaf(au, f.w, f.z);
-        b = fmaf(av, bot - top, top) - centre;
+    ok = ok && (ix < (unsigned)k.cam.Wm1) && (iy < (unsigned)k.cam.Hm1);
+    /* S4: one point fetch of the footprint + FP32 lerp (hardware texture filtering has 8-bit weights: too coarse for
+     * the 1e-4 cost tolerance).  Invalid samples fetch footprint 0 instead of branching around the load. */
+    float au = u - (tu - 12582912.f);
+    float av = v - (tv - 12582912.f);
+    const unsigned idx = ok ? iy * (unsigned)k.cam.W + ix : 0u;
+    float4 f;
+    if (F16) { /* 8-byte footprint of an 8-bit view: four bfloat16 (exact for integers up to 256) */
+        const uint2 w = __ldg(reinterpret_cast<const uint2*>(reinterpret_cast<const char*>(foot) + ((size_t)idx << 3)));
+        f.x = __uint_as_float(w.x << 16); f.y = __uint_as_float(w.x & 0xffff0000u);
+        f.z = __uint_as_float(w.y << 16); f.w = __uint_as_float(w.y & 0xffff0000u);
+    } else {
+        f = __ldg(reinterpret_cast<const float4*>(reinterpret_cast<const char*>(foot) + ((size_t)idx << 4)));
     }
-    return b;
+    float top = fmaf(au, f.y, f.x);
+    float bot = fmaf(au, f.w, f.z);
+    float b = fmaf(av, bot - top, top) - centre;
+    return ok ? b : CUDART_NAN_F;
 }
 
-/* 16 consecutive floats of a sample-plane row as 128-bit loads */
+/* NV4 * 4 consecutive floats of a sample-plane row as 128-bit loads */
 template <class G>
 __device__ __forceinline__ void load_run(const float* __restrict__ src, float (&p)[G::NV4 * 4]) {
     const float4* p4 = reinterpret_cast<const float4*>(src);
@@ -209,60 +225,73 @@ __device__ __forceinline__ void load_run(const float* __restrict__ src, float (&
 /* Horizontal pass of the separable box sums: one work item = RUN consecutive outputs of one halo row.
  * MODE 0: p = a', q = ray-valid flag      -> planes {sum a', sum a'^2, sum flag}
  * MODE 1: p = b', q = a' (all valid)      -> planes {sum b', sum b'^2, sum a'b'}
- * MODE 2: p = b' (NaN = invalid), q = a'  -> as MODE 1 with invalid samples as 0, plus plane 3 = sum valid */
+ * MODE 2: p = b' (NaN = invalid), q = a'  -> as MODE 1 with invalid samples as 0, plus plane 3 = sum valid;
+ *         returns whether any of the item's samples is valid
+ * The products enter and leave the sliding sums through FMAs (no product array is kept). */
 template <class G, int WIN, int MODE>
-__device__ __forceinline__ void hsum(float (&p)[G::NV4 * 4], const float (&q)[G::NV4 * 4], float* __restrict__ hs) {
+__device__ __forceinline__ bool hsum(float (&p)[G::NV4 * 4], const float (&q)[G::NV4 * 4], float* __restrict__ hs) {
     constexpr int NV = G::NV;
-    float okf[G::NV4 * 4];
+    float okf[MODE == 2 ? G::NV4 * 4 : 1];
+    bool any = true;
     if (MODE == 2) {
+        any = false;
 #pragma unroll
         for (int i = 0; i < NV; ++i) {
             bool ok = (p[i] == p[i]);
+            any = any || ok;
             okf[i] = ok ? 1.f : 0.f;
             p[i] = ok ? p[i] : 0.f;
         }
     }
-    float pp[G::NV4 * 4], pq[G::NV4 * 4];
-#pragma unroll
-    for (int i = 0; i < NV; ++i) {
-        pp[i] = p[i] * p[i];
-        pq[i] = (MODE == 0) ? q[i] : p[i] * q[i];
-    }
     float s0 = 0.f, s1 = 0.f, s2 = 0.f, s3 = 0.f;
 #pragma unroll
     for (int i = 0; i < WIN; ++i) {
-        s0 += p[i]; s1 += pp[i]; s2 += pq[i];
+        s0 += p[i];
+        s1 = fmaf(p[i], p[i], s1);
+        s2 = (MODE == 0) ? s2 + q[i] : fmaf(p[i], q[i], s2);
         if (MODE == 2) s3 += okf[i];
-    }
-    float o0[RUN], o1[RUN], o2[RUN], o3[RUN];
-    o0[0] = s0; o1[0] = s1; o2[0] = s2; o3[0] = s3;
-#pragma unroll
-    for (int j = 1; j < RUN; ++j) {
-        s0 += p[j + WIN - 1] - p[j - 1];
-        s1 += pp[j + WIN - 1] - pp[j - 1];
-        s2 += pq[j + WIN - 1] - pq[j - 1];
-        if (MODE == 2) s3 += okf[j + WIN - 1] - okf[j - 1];
-        o0[j] = s0; o1[j] = s1; o2[j] = s2; o3[j] = s3;
     }
     float4* h0 = reinterpret_cast<float4*>(hs);
     float4* h1 = reinterpret_cast<float4*>(hs + G::HPLANE);
     float4* h2 = reinterpret_cast<float4*>(hs + 2 * G::HPLANE);
-    h0[0] = make_float4(o0[0], o0[1], o0[2], o0[3]); h0[1] = make_float4(o0[4], o0[5], o0[6], o0[7]);
-    h1[0] = make_float4(o1[0], o1[1], o1[2], o1[3]); h1[1] = make_float4(o1[4], o1[5], o1[6], o1[7]);
-    h2[0] = make_float4(o2[0], o2[1], o2[2], o2[3]); h2[1] = make_float4(o2[4], o2[5], o2[6], o2[7]);
-    if (MODE == 2) {
-        float4* h3 = reinterpret_cast<float4*>(hs + 3 * G::HPLANE);
-        h3[0] = make_float4(o3[0], o3[1], o3[2], o3[3]); h3[1] = make_float4(o3[4], o3[5], o3[6], o3[7]);
+    float4* h3 = reinterpret_cast<float4*>(hs + 3 * G::HPLANE);
+    float o0[4], o1[4], o2[4], o3[4];
+#pragma unroll
+    for (int j = 0; j < RUN; ++j) {
+        if (j > 0) {
+            const int in = j + WIN - 1, out = j - 1;
+            s0 += p[in] - p[out];
+            s1 = fmaf(-p[out], p[out], fmaf(p[in], p[in], s1));
+            s2 = (MODE == 0) ? s2 + (q[in] - q[out]) : fmaf(-p[out], q[out], fmaf(p[in], q[in], s2));
+            if (MODE == 2) s3 += okf[in] - okf[out];
+        }
+        o0[j & 3] = s0; o1[j & 3] = s1; o2[j & 3] = s2; o3[j & 3] = s3;
+        if ((j & 3) == 3) {
+            h0[j >> 2] = make_float4(o0[0], o0[1], o0[2], o0[3]);
+            h1[j >> 2] = make_float4(o1[0], o1[1], o1[2], o1[3]);
+            h2[j >> 2] = make_float4(o2[0], o2[1], o2[2], o2[3]);
+            if (MODE == 2) h3[j >> 2] = make_float4(o3[0], o3[1], o3[2], o3[3]);
+        }
     }
+    return any;
 }
 
-/* Vertical pass: column x, output rows r0..r0+RPT-1; sums WIN consecutive row sums of one plane. */
+/* RUN entries of plane 3 (valid counts of the horizontal windows) of one work item set to c */
+template <class G>
+__device__ __forceinline__ void fill_count(float* __restrict__ hs, float c) {
+    float4* h3 = reinterpret_cast<float4*>(hs + 3 * G::HPLANE);
+    h3[0] = make_float4(c, c, c, c);
+    h3[1] = make_float4(c, c, c, c);
+}
+
+/* Vertical pass: h points at the first of the RPT + WIN - 1 row sums of this thread's column in one plane; sliding
+ * sums over WIN consecutive rows */
 template <class G, int WIN>
-__device__ __forceinline__ void vpass(const float* __restrict__ h, int x, int r0, float (&out)[G::RPT]) {
+__device__ __forceinline__ void vpass(const float* __restrict__ h, float (&out)[G::RPT]) {
     constexpr int RPT = G::RPT;
     float v[RPT + WIN - 1];
 #pragma unroll
-    for (int i = 0; i < RPT + WIN - 1; ++i) v[i] = h[(r0 + i) * G::HS + x];
+    for (int i = 0; i < RPT + WIN - 1; ++i) v[i] = h[i * G::HS];
     float s = 0.f;
 #pragma unroll
     for (int i = 0; i < WIN; ++i) s += v[i];
@@ -274,28 +303,32 @@ __device__ __forceinline__ void vpass(const float* __restrict__ h, int x, int r0
     }
 }
 
-/* streaming winner-take-all state of one output pixel (S7) */
+/* streaming winner-take-all state of one output pixel (S7).  b1 = lowest cost so far (lowest index wins ties),
+ * m2 = lowest cost of the planes at least two back (eligible as second best when the current plane becomes the
+ * best), s2 = second best of the current best, cm / cp = costs of the planes below / above the best, knext = index
+ * of the plane above the best while it is still to come in the same family. */
 struct Wta {
-    float b1, s2, m0, m1, cm, cp, cprev;
+    float b1, m2, s2, cm, cp, cprev;
     int k1, knext;
     __device__ __forceinline__ void init() {
-        b1 = CUDART_INF_F; s2 = CUDART_INF_F; m0 = CUDART_INF_F; m1 = CUDART_INF_F;
+        b1 = CUDART_INF_F; m2 = CUDART_INF_F; s2 = CUDART_INF_F;
         cm = CUDART_INF_F; cp = CUDART_INF_F; cprev = CUDART_INF_F;
         k1 = -1; knext = -1;
     }
     /* family start: planes of another family are never "adjacent" (reading Q12) */
-    __device__ __forceinline__ void family_start() { m1 = m0; cprev = CUDART_INF_F; knext = -1; }
+    __device__ __forceinline__ void family_start() { m2 = b1; cprev = CUDART_INF_F; knext = -1; }
     __device__ __forceinline__ void update(float c, int k) {
-        if (k == knext) cp = c;                 /* neighbour above the running best */
-        else if (k > knext) s2 = fminf(s2, c);  /* eligible second best */
-        if (c < b1) {                           /* strict: lowest index wins ties */
-            s2 = m1;                            /* best of everything at least two planes back */
-            cm = cprev;
-            cp = CUDART_INF_F;
-            b1 = c; k1 = k; knext = k + 1;
-        }
-        m1 = m0;
-        m0 = fminf(m0, c);
+        const bool isn = (k == knext);  /* neighbour above the running best: not eligible as second best */
+        const bool nb = c < b1;         /* strict: lowest index wins ties */
+        cp = isn ? c : cp;
+        const float t = isn ? s2 : fminf(s2, c);
+        s2 = nb ? m2 : t;
+        cm = nb ? cprev : cm;
+        cp = nb ? CUDART_INF_F : cp;
+        k1 = nb ? k : k1;
+        knext = nb ? k + 1 : knext;
+        m2 = b1;
+        b1 = fminf(b1, c);
         cprev = c;
     }
 };
@@ -306,36 +339,63 @@ __device__ __forceinline__ float warp_max(float v) {
     return v;
 }
 
-/* VC = views processed together (1 or 2); args.n_views > VC runs the views in chunks of VC.
- * ONECHUNK: args.n_views <= VC, so that view indices are compile-time constants. */
-template <int WIN, int VC, bool ONECHUNK, bool IDENT, bool FULLDIST, bool CHECKDEN, class G>
-__global__ void __launch_bounds__(G::NT, G::MINB) sweep_kernel(const __grid_constant__ FswSweepArgs args) {
-    constexpr int HW = G::HW, RPT = G::RPT, NT = G::NT, NS = G::NS, TX = G::TX, TY = G::TY;
+/* horizontal work item of lane `lane`: local row (0..R-1, or -1 for an idle lane) and run (0..7).  A quarter-warp
+ * covers rows {r, r+1} x four runs: its 128-bit stores into the row-sum planes (row stride == 4 mod 8 words) hit
+ * eight distinct 16-byte bank groups. */
+template <class G>
+__device__ __forceinline__ void h_item(int lane, int& row, int& run) {
+    const int half = lane >> 4, l = lane & 15;
+    row = 2 * half + ((l >> 2) & 1);
+    run = (l & 3) + ((l >> 3) << 2);
+    if (G::R == 3 && half == 1) { /* third row: eight runs in lanes 16..23, lanes 24..31 idle */
+        row = l < 8 ? 2 : -1;
+        run = l & 7;
+    }
+}
+
+/* the fields of a frame set the sweep loop touches, staged in shared memory once per tile */
+struct SetHot {
+    const void* foot[FSW_MAX_VIEWS];
+    float* debug_cost;
+};
+
+/* NVT = number of views known at compile time (1 or 2), 0 = read args.n_views at run time. */
+template <int WIN, int NVT, bool IDENT, bool FULLDIST, bool CHECKDEN, bool F16>
+__global__ void __launch_bounds__(Geo<WIN>::NT, 1) sweep_kernel(const __grid_constant__ FswSweepArgs args) {
+    using G = Geo<WIN>;
+    constexpr int HW = G::HW, RPT = G::RPT, NS = G::NS, TX = G::TX, TY = G::TY, R = G::R;
     constexpr float NWIN = (float)(WIN * WIN);
     constexpr float INV_NWIN = 1.f / NWIN;
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    float4* rays = reinterpret_cast<float4*>(smem_raw);
-    float* a_s = reinterpret_cast<float*>(rays + G::PLANE);
-    float* b_s = a_s + G::PLANE;          /* [VC][PLANE] */
-    float* hs = b_s + VC * G::PLANE;      /* [VC][4][HPLANE] */
+    float4* rays = reinterpret_cast<float4*>(smem_raw);   /* [EHA][SB]: unit ray, .w = validity / incidence */
+    float* a_s = reinterpret_cast<float*>(rays + G::PLANE); /* [EHA][SB]: centred reference intensities a' */
+    float* b_s = a_s + G::PLANE;                           /* [EHA][SB]: samples b' of the current (plane, view) */
+    float* hs = b_s + G::PLANE;                            /* [4][EHA][HS]: row sums */
     __shared__ float red_f[G::NW];
     __shared__ int red_i[G::NW];
-    __shared__ unsigned s_flags[2][2];    /* [parity][0: AND of "all valid" bits, 1: OR of "any valid" bits] */
+    __shared__ unsigned s_mixed[3], s_any[3]; /* rotating flags of a (plane, view) pass */
     __shared__ unsigned s_item;
+    __shared__ SetHot s_set;
 
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     const int col = tid % TX, grp = tid / TX;
     const int W = args.ref.W, H = args.ref.H;
     const int n_items = args.n_tiles * args.n_sets;
+    const int n_views = NVT ? NVT : args.n_views;
 
-    /* this thread's halo pixels: logical index -> offset in the padded sample planes */
-    int soff[NS];
-#pragma unroll
-    for (int i = 0; i < NS; ++i) {
-        int idx = tid + i * NT;
-        int row = idx / G::EW;
-        soff[i] = idx < G::NE ? row * G::SB + (idx - row * G::EW) : -1;
-    }
+    /* this lane's halo pixels: slot i is element lane + 32 i of the warp's R x SB block of the sample planes; in the
+     * last slot only the lanes below `tail` have a pixel */
+    const int sbase = wid * R * G::SB + lane;
+    constexpr int TAIL = R * G::SB - 32 * G::NSFULL; /* 0 if every slot is full */
+    const bool tail_on = lane < TAIL;
+    /* this lane's horizontal work item */
+    int hrow_l, hrun;
+    h_item<G>(lane, hrow_l, hrun);
+    const int hrow = wid * R + hrow_l;
+    const bool h_on = hrow_l >= 0 && hrow < G::EH;
+    const int h_src = h_on ? hrow * G::SB + hrun * RUN : 0;
+    float* const h_dst = hs + (h_on ? hrow * G::HS + hrun * RUN : 0);
+    const float* const v_src = hs + (grp * RPT) * G::HS + col; /* first row sum of this thread's vertical pass */
 
     unsigned item = blockIdx.x;
     while (item < (unsigned)n_items) {
@@ -365,17 +425,24 @@ __global__ void __launch_bounds__(G::NT, G::MINB) sweep_kernel(const __grid_cons
 #pragma unroll
         for (int i = 0; i < RPT; ++i) { A1n[i] = 0.f; A2[i] = 0.f; }
         float centre = 0.f;
+        float areg[G::NV4 * 4];   /* a' operands of this lane's horizontal work item */
+#pragma unroll
+        for (int i = 0; i < G::NV4 * 4; ++i) areg[i] = 0.f;
+        int p3 = 0;               /* state of this warp's rows of plane 3: 0 = WIN everywhere, 1 = zero, 2 = counts */
+        const bool dbg = S.debug_cost != nullptr;
 
         if (tile_live) {
+            if (tid < FSW_MAX_VIEWS) s_set.foot[tid] = S.foot[tid];
+            if (tid == 32) s_set.debug_cost = S.debug_cost;
             /* ---- S1: rays and reference intensities of the tile + halo ------------------------------------ */
             float lsum = 0.f;
             int lcnt = 0;
 #pragma unroll 1
             for (int i = 0; i < NS; ++i) {
-                int idx = tid + i * NT;
-                if (idx >= G::NE) break;
-                int row = idx / G::EW, cx_ = idx - row * G::EW;
-                int px = x0t - HW + cx_, py = y0t - HW + row;
+                const int p = lane + 32 * i;
+                if (p >= R * G::SB) break;
+                const int lr = p / G::SB, cx_ = p - lr * G::SB, row = wid * R + lr;
+                const int px = x0t - HW + cx_, py = y0t - HW + row;
                 float4 ry = make_float4(0.f, 0.f, 0.f, 0.f); /* invalid rays are zero vectors */
                 float a = 0.f;
                 if (px >= 0 && px < W && py >= 0 && py < H) {
@@ -388,7 +455,7 @@ __global__ void __launch_bounds__(G::NT, G::MINB) sweep_kernel(const __grid_cons
                         a = __ldg(reinterpret_cast<const float*>(reinterpret_cast<const char*>(S.ref_img) + (int64_t)py * S.ref_pitch_bytes) + px);
                     if (ok) { lsum += a; lcnt += 1; } /* pixels outside the FOV never enter a valid window */
                 }
-                int o = row * G::SB + cx_;
+                const int o = sbase + 32 * i;
                 rays[o] = ry;
                 a_s[o] = a;
                 b_s[o] = ry.w;
@@ -410,22 +477,24 @@ __global__ void __launch_bounds__(G::NT, G::MINB) sweep_kernel(const __grid_cons
             if (S.ref_dtype == FSW_U8) centre = rintf(centre);
 #pragma unroll
             for (int i = 0; i < NS; ++i)
-                if (soff[i] >= 0) a_s[soff[i]] -= centre;
-            __syncthreads();
-            /* window sums of the reference side, once per pixel */
-            for (int it = tid; it < G::NHITEM; it += NT) {
-                const int run = it / G::EH, row = it - run * G::EH;
-                float p[G::NV4 * 4], q[G::NV4 * 4];
-                load_run<G>(a_s + row * G::SB + run * RUN, p);
-                load_run<G>(b_s + row * G::SB + run * RUN, q);
-                hsum<G, WIN, 0>(p, q, hs + row * G::HS + run * RUN);
+                if (i < G::NSFULL || tail_on) a_s[sbase + 32 * i] -= centre;
+            __syncwarp();
+            /* window sums of the reference side, once per pixel; the a' run stays in registers */
+            if (h_on) {
+                float q[G::NV4 * 4], p[G::NV4 * 4];
+                load_run<G>(a_s + h_src, areg);
+                load_run<G>(b_s + h_src, q);
+#pragma unroll
+                for (int i = 0; i < G::NV4 * 4; ++i) p[i] = areg[i];
+                hsum<G, WIN, 0>(p, q, h_dst);
+                fill_count<G>(h_dst, (float)WIN);
             }
             __syncthreads();
             {
                 float sa[RPT], saa[RPT], sf[RPT];
-                vpass<G, WIN>(hs, col, grp * RPT, sa);
-                vpass<G, WIN>(hs + G::HPLANE, col, grp * RPT, saa);
-                vpass<G, WIN>(hs + 2 * G::HPLANE, col, grp * RPT, sf);
+                vpass<G, WIN>(v_src, sa);
+                vpass<G, WIN>(v_src + G::HPLANE, saa);
+                vpass<G, WIN>(v_src + 2 * G::HPLANE, sf);
 #pragma unroll
                 for (int i = 0; i < RPT; ++i) {
                     int oy = oy0 + i;
@@ -436,36 +505,37 @@ __global__ void __launch_bounds__(G::NT, G::MINB) sweep_kernel(const __grid_cons
                     A2[i] = fmaf(-A1n[i], sa[i], saa[i]);
                 }
             }
-            if (tid == 0) { s_flags[0][0] = ~0u; s_flags[0][1] = 0u; s_flags[1][0] = ~0u; s_flags[1][1] = 0u; }
+            if (tid == 0) { s_mixed[0] = 0u; s_mixed[1] = 0u; s_mixed[2] = 0u; s_any[0] = 0u; s_any[1] = 0u; s_any[2] = 0u; }
             tile_active = __syncthreads_or(active_mask != 0) != 0;
         }
 
         if (tile_active) {
-            const float inv_views = 1.f / (float)args.n_views;
-            unsigned parity = 0;
+            const float inv_views = 1.f / (float)n_views;
+            unsigned ph = 0; /* rotation of the pass flags */
 #pragma unroll 1
             for (int f = 0; f < args.n_fams; ++f) {
                 const FswDevFamily& F = args.fam[f];
                 const float fnx = F.n[0], fny = F.n[1], fnz = F.n[2];
 #pragma unroll
                 for (int i = 0; i < RPT; ++i) st[i].family_start();
-                /* incidence q = n.r of every halo ray with this family, NaN where the ray does not face the planes
-                 * (or is outside the camera); q_max decides which planes can be reached within range_max */
-                float qmax = 0.f;
+                /* incidence q = n.r of this lane's halo rays with the family, NaN where the ray does not face the
+                 * planes (or is outside the camera); the largest q of the warp's rows / of the tile decides which
+                 * planes can be reached within range_max */
+                float qmax_w = 0.f;
 #pragma unroll
                 for (int i = 0; i < NS; ++i) {
-                    if (soff[i] < 0) continue;
-                    float4 ry = rays[soff[i]];
+                    if (i >= G::NSFULL && !tail_on) continue;
+                    float4 ry = rays[sbase + 32 * i];
                     float q = fmaf(fnx, ry.x, fmaf(fny, ry.y, fnz * ry.z));
                     bool faces = q > FSW_EPS_Q; /* an invalid reference ray is the zero vector: q = 0 */
-                    rays[soff[i]].w = faces ? q : CUDART_NAN_F;
-                    if (faces) qmax = fmaxf(qmax, q);
+                    rays[sbase + 32 * i].w = faces ? q : CUDART_NAN_F;
+                    if (faces) qmax_w = fmaxf(qmax_w, q);
                 }
-                qmax = warp_max(qmax);
+                qmax_w = warp_max(qmax_w);
                 __syncthreads(); /* previous users of red_f are done */
-                if (lane == 0) red_f[wid] = qmax;
+                if (lane == 0) red_f[wid] = qmax_w;
                 __syncthreads();
-                qmax = 0.f;
+                float qmax = 0.f;
 #pragma unroll
                 for (int i = 0; i < G::NW; ++i) qmax = fmaxf(qmax, red_f[i]);
 
@@ -474,87 +544,87 @@ __global__ void __launch_bounds__(G::NT, G::MINB) sweep_kernel(const __grid_cons
                     const int k = F.first + j;
                     const float inv_d = args.inv_d[k];
                     float acc[RPT];
-                    int cnt[RPT];
+                    unsigned cnt = 0; /* valid views per output, 4 bits each */
 #pragma unroll
-                    for (int i = 0; i < RPT; ++i) { acc[i] = 0.f; cnt[i] = 0; }
+                    for (int i = 0; i < RPT; ++i) acc[i] = 0.f;
                     /* S2: the plane is out of reach for the whole tile if even the best-facing ray is beyond range */
-                    const bool plane_on = qmax * inv_d >= args.inv_range_max;
-                    if (plane_on) {
+                    if (qmax * inv_d >= args.inv_range_max) {
+                        const bool rows_on = qmax_w * inv_d >= args.inv_range_max; /* any ray of this warp's rows */
+                        constexpr int VSTEP = NVT ? NVT : 1;
 #pragma unroll 1
-                        for (int v0 = 0; v0 < (ONECHUNK ? 1 : args.n_views); v0 += VC) {
-                            /* ---- S2-S4: sample the plane-warped views at every halo pixel ------------------- */
-                            bool all_ok[VC], any_ok[VC];
+                        for (int v0 = 0; v0 < n_views; v0 += VSTEP) {
 #pragma unroll
-                            for (int v = 0; v < VC; ++v) { all_ok[v] = true; any_ok[v] = false; }
+                            for (int vv = 0; vv < VSTEP; ++vv) {
+                                const int v = v0 + vv;
+                                /* ---- S2-S4: sample the plane-warped view at this warp's halo rows ------------- */
+                                bool all_ok = true;
+                                if (rows_on) {
+                                    const void* fv = s_set.foot[v];
 #pragma unroll
-                            for (int i = 0; i < NS; ++i) {
-                                if (soff[i] < 0) continue;
-                                const float4 ry = rays[soff[i]];
-                                float s = ry.w * inv_d;
-                                s = (s >= args.inv_range_max) ? s : CUDART_NAN_F;
-#pragma unroll
-                                for (int v = 0; v < VC; ++v) {
-                                    if (!ONECHUNK && v0 + v >= args.n_views) break;
-                                    const int vi = ONECHUNK ? v : v0 + v;
-                                    float b = warp_sample<IDENT, FULLDIST, CHECKDEN>(ry.x, ry.y, ry.z, s, args.views[vi], S.foot[vi], centre);
-                                    b_s[v * G::PLANE + soff[i]] = b;
-                                    bool okb = (b == b);
-                                    all_ok[v] = all_ok[v] && okb;
-                                    any_ok[v] = any_ok[v] || okb;
+                                    for (int i = 0; i < NS; ++i) {
+                                        if (i >= G::NSFULL && !tail_on) continue;
+                                        const float4 ry = rays[sbase + 32 * i];
+                                        float s = ry.w * inv_d;
+                                        s = (s >= args.inv_range_max) ? s : CUDART_NAN_F;
+                                        bool ok;
+                                        float b = warp_sample<IDENT, FULLDIST, CHECKDEN, F16>(ry.x, ry.y, ry.z, s, args.views[v], fv, centre, ok);
+                                        b_s[sbase + 32 * i] = b;
+                                        all_ok = all_ok && ok;
+                                    }
+                                    all_ok = __all_sync(0xffffffffu, all_ok);
                                 }
-                            }
-                            unsigned fl_all = 0, fl_any = 0;
-#pragma unroll
-                            for (int v = 0; v < VC; ++v) {
-                                if (__all_sync(0xffffffffu, all_ok[v])) fl_all |= 1u << v;
-                                if (__any_sync(0xffffffffu, any_ok[v])) fl_any |= 1u << v;
-                            }
-                            if (lane == 0) {
-                                atomicAnd(&s_flags[parity][0], fl_all);
-                                atomicOr(&s_flags[parity][1], fl_any);
-                            }
-                            __syncthreads(); /* [A] */
-                            const unsigned f_all = s_flags[parity][0], f_any = s_flags[parity][1];
-                            if (tid == 0) { s_flags[parity ^ 1][0] = ~0u; s_flags[parity ^ 1][1] = 0u; }
-                            parity ^= 1;
-                            if (f_any == 0) continue; /* no view sees anything of the tile through this plane */
-                            /* ---- S5: separable box sums ----------------------------------------------------- */
-                            for (int it = tid; it < G::NHITEM; it += NT) {
-                                const int run = it / G::EH, row = it - run * G::EH;
-                                float q[G::NV4 * 4];
-                                load_run<G>(a_s + row * G::SB + run * RUN, q);
-#pragma unroll
-                                for (int v = 0; v < VC; ++v) {
-                                    if (!((f_any >> v) & 1u)) continue;
-                                    float p[G::NV4 * 4];
-                                    load_run<G>(b_s + v * G::PLANE + row * G::SB + run * RUN, p);
-                                    float* dst = hs + v * 4 * G::HPLANE + row * G::HS + run * RUN;
-                                    if ((f_all >> v) & 1u) hsum<G, WIN, 1>(p, q, dst);
-                                    else hsum<G, WIN, 2>(p, q, dst);
+                                __syncwarp();
+                                /* ---- S5: horizontal box sums of the same rows --------------------------------- */
+                                bool any_ok = rows_on;
+                                if (rows_on) {
+                                    bool any_l = false;
+                                    if (h_on) {
+                                        float p[G::NV4 * 4];
+                                        load_run<G>(b_s + h_src, p);
+                                        if (!G::A_IN_REGS) load_run<G>(a_s + h_src, areg);
+                                        if (all_ok) {
+                                            hsum<G, WIN, 1>(p, areg, h_dst);
+                                            if (p3 != 0) fill_count<G>(h_dst, (float)WIN);
+                                        } else {
+                                            any_l = hsum<G, WIN, 2>(p, areg, h_dst);
+                                        }
+                                    }
+                                    if (!all_ok) any_ok = __any_sync(0xffffffffu, any_l);
+                                    p3 = all_ok ? 0 : 2;
+                                } else {
+                                    if (p3 != 1 && h_on) fill_count<G>(h_dst, 0.f);
+                                    p3 = 1;
                                 }
-                            }
-                            __syncthreads(); /* [B] */
-                            /* ---- ZNCC ----------------------------------------------------------------------- */
-#pragma unroll
-                            for (int v = 0; v < VC; ++v) {
-                                if (!((f_any >> v) & 1u)) continue;
-                                const bool mixed = !((f_all >> v) & 1u);
-                                const float* hv = hs + v * 4 * G::HPLANE;
+                                if (lane == 0) {
+                                    if (any_ok) s_any[ph] = 1u;
+                                    if (!(rows_on && all_ok)) s_mixed[ph] = 1u;
+                                }
+                                __syncthreads(); /* [A] row sums of the pass are complete */
+                                const unsigned f_mixed = s_mixed[ph], f_any = s_any[ph];
+                                {
+                                    const unsigned nx = ph >= 1 ? ph - 1 : 2; /* (ph + 2) % 3: the flags after next */
+                                    if (tid == 0) { s_mixed[nx] = 0u; s_any[nx] = 0u; }
+                                }
+                                ph = ph == 2 ? 0 : ph + 1;
+                                if (f_any == 0) continue; /* the view sees nothing of the tile through this plane */
+                                /* ---- vertical sums, ZNCC ------------------------------------------------------ */
                                 float sb[RPT], sbb[RPT], sab[RPT], sv[RPT];
-                                vpass<G, WIN>(hv, col, grp * RPT, sb);
-                                vpass<G, WIN>(hv + G::HPLANE, col, grp * RPT, sbb);
-                                vpass<G, WIN>(hv + 2 * G::HPLANE, col, grp * RPT, sab);
-                                if (mixed) vpass<G, WIN>(hv + 3 * G::HPLANE, col, grp * RPT, sv);
+                                vpass<G, WIN>(v_src, sb);
+                                vpass<G, WIN>(v_src + G::HPLANE, sbb);
+                                vpass<G, WIN>(v_src + 2 * G::HPLANE, sab);
+                                if (f_mixed) vpass<G, WIN>(v_src + 3 * G::HPLANE, sv);
+                                __syncthreads(); /* [B] everyone has read the row sums: the next pass may overwrite */
 #pragma unroll
                                 for (int i = 0; i < RPT; ++i) {
                                     bool okv = (active_mask >> i) & 1u;
-                                    if (mixed) okv = okv && (sv[i] == NWIN);
+                                    if (f_mixed) okv = okv && (sv[i] == NWIN);
                                     float cov = fmaf(-A1n[i], sb[i], sab[i]);
                                     float vb = fmaf(-sb[i] * INV_NWIN, sb[i], sbb[i]);
                                     float prod = fmaxf(A2[i] * vb, args.floor2);
                                     float z = cov * rsqrt_approx(prod);
                                     float cst = __saturatef(fmaf(-0.5f, z, 0.5f));
-                                    if (okv) { acc[i] += cst; cnt[i] += 1; }
+                                    acc[i] += okv ? cst : 0.f;
+                                    cnt += okv ? (1u << (4 * i)) : 0u;
                                 }
                             }
                         }
@@ -562,20 +632,27 @@ __global__ void __launch_bounds__(G::NT, G::MINB) sweep_kernel(const __grid_cons
                     /* ---- S6 + S7: view mean, streaming winner-take-all ------------------------------------- */
 #pragma unroll
                     for (int i = 0; i < RPT; ++i) {
-                        float c = CUDART_INF_F;
-                        if (cnt[i] == args.n_views) c = acc[i] * inv_views;
-                        else if (cnt[i] > 0) c = acc[i] / (float)cnt[i];
-                        n_eval += cnt[i];
-                        if (S.debug_cost != nullptr) {
-                            int oy = oy0 + i;
-                            if (ox < W && oy < H) S.debug_cost[((int64_t)k * H + oy) * W + ox] = c;
-                        }
+                        const int ci = (int)((cnt >> (4 * i)) & 15u);
+                        float c;
+                        if (NVT == 1) c = acc[i];
+                        else if (NVT == 2) c = ci == 2 ? 0.5f * acc[i] : acc[i];
+                        else c = ci == n_views ? acc[i] * inv_views : acc[i] * args.inv_count[ci];
+                        c = ci > 0 ? c : CUDART_INF_F;
+                        n_eval += ci;
                         st[i].update(c, k);
+                    }
+                    if (dbg) {
+                        float* dc = s_set.debug_cost;
+#pragma unroll
+                        for (int i = 0; i < RPT; ++i) {
+                            const int oy = oy0 + i;
+                            if (ox < W && oy < H) dc[((int64_t)k * H + oy) * W + ox] = st[i].cprev;
+                        }
                     }
                 }
             }
         }
-        if (S.debug_cost != nullptr && !tile_active) {
+        if (dbg && !tile_active) {
             for (int k = 0; k < args.n_planes; ++k)
 #pragma unroll
                 for (int i = 0; i < RPT; ++i) {
@@ -665,55 +742,63 @@ __global__ void __launch_bounds__(G::NT, G::MINB) sweep_kernel(const __grid_cons
     }
 }
 
-/* The tile shapes: A = 64x32 outputs, 512 threads, one CTA per SM (windows up to 9);
- *                  B = 32x32 outputs, 256 threads (larger windows: the halo planes of A would not fit). */
-template <int WIN> struct GeoFor { using type = Geo<WIN, 64, 32, 512, 1>; };
-template <> struct GeoFor<11> { using type = Geo<11, 32, 32, 256, 1>; };
-template <> struct GeoFor<13> { using type = Geo<13, 32, 32, 256, 1>; };
-template <> struct GeoFor<15> { using type = Geo<15, 32, 32, 256, 1>; };
-
-/* Kernel variants: 0 = generic (any rotation, full distortion polynomial, denominator test),
- *                  1 = identity rotations, k1-only (or no) distortion, cos(fov/2) + xi >= 1e-3. */
-template <int WIN, int VC, bool ONE>
+/* Kernel variants: bit 0 = identity rotations, k1-only (or no) distortion, cos(fov/2) + xi >= 1e-3 (otherwise any
+ * rotation, the full distortion polynomial and the denominator test); bit 1 = 8-byte bfloat16 footprints. */
+template <int WIN, int NVT>
 struct SweepInst {
-    using G = typename GeoFor<WIN>::type;
-    static cudaError_t launch(const FswSweepArgs& args, int variant, int grid, cudaStream_t stream) {
-        const size_t smem = G::smem(VC);
-        if (variant == 1) sweep_kernel<WIN, VC, ONE, true, false, false, G><<<grid, G::NT, smem, stream>>>(args);
-        else sweep_kernel<WIN, VC, ONE, false, true, true, G><<<grid, G::NT, smem, stream>>>(args);
+    using G = Geo<WIN>;
+    template <bool FAST, bool F16>
+    static cudaError_t go(const FswSweepArgs& args, int grid, cudaStream_t stream, bool prepare_only) {
+        auto kern = sweep_kernel<WIN, NVT, FAST, !FAST, !FAST, F16>;
+        if (prepare_only) return cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::smem());
+        kern<<<grid, G::NT, G::smem(), stream>>>(args);
         return cudaGetLastError();
     }
+    static cudaError_t dispatch(const FswSweepArgs& args, int variant, int grid, cudaStream_t stream, bool prep) {
+        switch (variant & 3) {
+            case 0: return go<false, false>(args, grid, stream, prep);
+            case 1: return go<true, false>(args, grid, stream, prep);
+            case 2: return go<false, true>(args, grid, stream, prep);
+            default: return go<true, true>(args, grid, stream, prep);
+        }
+    }
+    static cudaError_t launch(const FswSweepArgs& args, int variant, int grid, cudaStream_t stream) {
+        return dispatch(args, variant, grid, stream, false);
+    }
     static cudaError_t prepare() {
-        const int smem = (int)G::smem(VC);
-        cudaError_t e = cudaFuncSetAttribute(sweep_kernel<WIN, VC, ONE, true, false, false, G>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-        if (e != cudaSuccess) return e;
-        return cudaFuncSetAttribute(sweep_kernel<WIN, VC, ONE, false, true, true, G>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        static const FswSweepArgs dummy = {};
+        for (int v = 0; v < 4; ++v) {
+            cudaError_t e = dispatch(dummy, v, 0, nullptr, true);
+            if (e != cudaSuccess) return e;
+        }
+        return cudaSuccess;
     }
 };
 
-/* n_views == 1 -> VC = 1; n_views == 2 -> VC = 2, one chunk; more views -> chunks of 2 */
+/* one or two views: the view loop is unrolled; more: a run-time loop */
 template <int WIN>
 cudaError_t launch_sweep_win(const FswSweepArgs& args, int variant, int grid, cudaStream_t stream) {
-    if (args.n_views == 1) return SweepInst<WIN, 1, true>::launch(args, variant, grid, stream);
-    if (args.n_views == 2) return SweepInst<WIN, 2, true>::launch(args, variant, grid, stream);
-    return SweepInst<WIN, 2, false>::launch(args, variant, grid, stream);
+    if (args.n_views == 1) return SweepInst<WIN, 1>::launch(args, variant, grid, stream);
+    if (args.n_views == 2) return SweepInst<WIN, 2>::launch(args, variant, grid, stream);
+    return SweepInst<WIN, 0>::launch(args, variant, grid, stream);
 }
 
 template <int WIN>
 cudaError_t prepare_sweep_win() {
-    cudaError_t e = SweepInst<WIN, 1, true>::prepare();
+    cudaError_t e = SweepInst<WIN, 1>::prepare();
     if (e != cudaSuccess) return e;
-    e = SweepInst<WIN, 2, true>::prepare();
+    e = SweepInst<WIN, 2>::prepare();
     if (e != cudaSuccess) return e;
-    return SweepInst<WIN, 2, false>::prepare();
+    return SweepInst<WIN, 0>::prepare();
 }
 
 template <int WIN>
 FswSweepGeometry geometry_win(int n_views) {
-    using G = typename GeoFor<WIN>::type;
+    using G = Geo<WIN>;
+    (void)n_views;
     FswSweepGeometry g;
     g.tile_w = G::TX; g.tile_h = G::TY; g.threads = G::NT; g.ctas_per_sm = G::MINB;
-    g.smem_bytes = G::smem(n_views == 1 ? 1 : 2);
+    g.smem_bytes = G::smem();
     return g;
 }
 
