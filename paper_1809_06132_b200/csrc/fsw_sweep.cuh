@@ -34,6 +34,7 @@
 #define FSW_SWEEP_CUH
 
 #include <math_constants.h>
+#include <cstdio>
 
 #include "fsw_internal.h"
 
@@ -144,16 +145,20 @@ __device__ inline bool back_project(const FswDevCam& c, float u, float v, float&
     return rz >= c.cos_fov; /* theta <= fov/2 */
 }
 
-/* S3-S4 for one halo pixel and one view: bilinear sample of the view at the plane-induced position minus `centre`;
- * `ok` is false (and the value NaN) if the pixel / plane / view combination is invalid ("NONE" of SURVEY 8(b)).
+/* S2-S3 for one halo pixel and one view: where the plane-induced position falls in the view (footprint index and
+ * bilinear weights); `ok` is false if the pixel / plane / view combination is invalid ("NONE" of SURVEY 8(b)).
  * (rx,ry,rz) is the reference ray, s = (n.r)/d_k the inverse range along it (NaN if the ray misses the plane or the
  * intersection is beyond range_max: the NaN then fails the field-of-view test below, no separate flag is carried).
  * IDENT: the view's relative rotation is the identity.  FULLDIST: k2 / p1 / p2 may be non-zero.
  * CHECKDEN: cos(fov/2) + xi may be < 1e-3, so the projection denominator is tested on its own.
  * F16: the footprint images hold four bfloat16 per pixel (8-bit views) instead of four floats. */
-template <bool IDENT, bool FULLDIST, bool CHECKDEN, bool F16>
-__device__ __forceinline__ float warp_sample(float rx, float ry, float rz, float s, const FswDevView& k,
-                                             const void* __restrict__ foot, float centre, bool& ok) {
+struct SampleAddr {
+    float au, av;  /* bilinear weights */
+    unsigned idx;  /* footprint index iy * W + ix, 0 for an invalid sample */
+    bool ok;
+};
+template <bool IDENT, bool FULLDIST, bool CHECKDEN>
+__device__ __forceinline__ SampleAddr sample_addr(float rx, float ry, float rz, float s, const FswDevView& k) {
     /* S2: X' ~ R r + s T */
     float X, Y, Z;
     if (IDENT) {
@@ -169,7 +174,7 @@ __device__ __forceinline__ float warp_sample(float rx, float ry, float rz, float
     float rho2 = fmaf(X, X, fmaf(Y, Y, Z * Z));
     float irho = rsqrt_approx(rho2);
     float t = fmaf(Z, irho, k.cam.xi);       /* cos(theta) + xi; NaN for rho2 == 0 */
-    ok = t >= k.cam.cos_fov_xi;              /* theta <= fov/2; false for NaN */
+    bool ok = t >= k.cam.cos_fov_xi;         /* theta <= fov/2; false for NaN */
     if (CHECKDEN) ok = ok && (t > FSW_EPS_DEN);
     float g = irho * rcp_approx(t);
     float mx = X * g, my = Y * g;
@@ -192,18 +197,39 @@ __device__ __forceinline__ float warp_sample(float rx, float ry, float rz, float
     unsigned ix = (unsigned)__float_as_int(tu) - 0x4B400000u, iy = (unsigned)__float_as_int(tv) - 0x4B400000u;
     /* bilinear footprint inside the view image: 0 <= u < W-1, 0 <= v < H-1  <=>  0 <= floor(u) < W-1, ... */
     ok = ok && (ix < (unsigned)k.cam.Wm1) && (iy < (unsigned)k.cam.Hm1);
-    /* S4: one point fetch of the footprint + FP32 lerp (hardware texture filtering has 8-bit weights: too coarse for
-     * the 1e-4 cost tolerance).  Invalid samples fetch footprint 0 instead of branching around the load. */
-    float au = u - (tu - 12582912.f);
-    float av = v - (tv - 12582912.f);
-    const unsigned idx = ok ? iy * (unsigned)k.cam.W + ix : 0u;
+    SampleAddr a;
+    a.au = u - (tu - 12582912.f);
+    a.av = v - (tv - 12582912.f);
+    a.idx = ok ? iy * (unsigned)k.cam.W + ix : 0u; /* invalid samples fetch footprint 0 instead of branching */
+#ifdef FSW_DEBUG_CLAMP
+    a.idx = min(a.idx, (unsigned)(k.cam.W * k.cam.H - 1));
+#endif
+#ifdef FSW_DEBUG_BOUNDS
+    if (a.idx >= (unsigned)(k.cam.W * k.cam.H)) { printf("bad idx %u ix %u iy %u ok %d W %d H %d\n", a.idx, ix, iy, (int)ok, k.cam.W, k.cam.H); a.idx = 0; }
+#endif
+    a.ok = ok;
+    return a;
+}
+
+/* S4: one point fetch of the footprint + FP32 lerp (hardware texture filtering has 8-bit weights: too coarse for the
+ * 1e-4 cost tolerance).  Raw footprint: 8 bytes = four bfloat16 (F16, exact for integers up to 256) or four floats. */
+template <bool F16> struct FootRaw { float4 v; };
+template <> struct FootRaw<true> { uint2 v; };
+template <bool F16>
+__device__ __forceinline__ FootRaw<F16> foot_fetch(const void* __restrict__ foot, unsigned idx) {
+    FootRaw<F16> r;
+    if constexpr (F16) r.v = __ldg(reinterpret_cast<const uint2*>(reinterpret_cast<const char*>(foot) + ((size_t)idx << 3)));
+    else r.v = __ldg(reinterpret_cast<const float4*>(reinterpret_cast<const char*>(foot) + ((size_t)idx << 4)));
+    return r;
+}
+template <bool F16>
+__device__ __forceinline__ float foot_lerp(const FootRaw<F16>& r, float au, float av, bool ok, float centre) {
     float4 f;
-    if (F16) { /* 8-byte footprint of an 8-bit view: four bfloat16 (exact for integers up to 256) */
-        const uint2 w = __ldg(reinterpret_cast<const uint2*>(reinterpret_cast<const char*>(foot) + ((size_t)idx << 3)));
-        f.x = __uint_as_float(w.x << 16); f.y = __uint_as_float(w.x & 0xffff0000u);
-        f.z = __uint_as_float(w.y << 16); f.w = __uint_as_float(w.y & 0xffff0000u);
+    if constexpr (F16) {
+        f.x = __uint_as_float(r.v.x << 16); f.y = __uint_as_float(r.v.x & 0xffff0000u);
+        f.z = __uint_as_float(r.v.y << 16); f.w = __uint_as_float(r.v.y & 0xffff0000u);
     } else {
-        f = __ldg(reinterpret_cast<const float4*>(reinterpret_cast<const char*>(foot) + ((size_t)idx << 4)));
+        f = r.v;
     }
     float top = fmaf(au, f.y, f.x);
     float bot = fmaf(au, f.w, f.z);
@@ -366,6 +392,10 @@ __global__ void __launch_bounds__(Geo<WIN>::NT, 1) sweep_kernel(const __grid_con
     constexpr int HW = G::HW, RPT = G::RPT, NS = G::NS, TX = G::TX, TY = G::TY, R = G::R;
     constexpr float NWIN = (float)(WIN * WIN);
     constexpr float INV_NWIN = 1.f / NWIN;
+#ifndef FSW_SBATCH
+#define FSW_SBATCH 4
+#endif
+    constexpr int SBATCH = FSW_SBATCH; /* samples in flight per lane */
     extern __shared__ __align__(16) unsigned char smem_raw[];
     float4* rays = reinterpret_cast<float4*>(smem_raw);   /* [EHA][SB]: unit ray, .w = validity / incidence */
     float* a_s = reinterpret_cast<float*>(rays + G::PLANE); /* [EHA][SB]: centred reference intensities a' */
@@ -560,16 +590,46 @@ __global__ void __launch_bounds__(Geo<WIN>::NT, 1) sweep_kernel(const __grid_con
                                 bool all_ok = true;
                                 if (rows_on) {
                                     const void* fv = s_set.foot[v];
+#ifdef FSW_DEBUG_BOUNDS
+                                    if (fv == nullptr || v >= args.n_views) printf("bad foot v %d %p\n", v, fv);
+#endif
+                                    /* batches of SBATCH samples: all addresses, then all fetches, then the lerps */
 #pragma unroll
-                                    for (int i = 0; i < NS; ++i) {
-                                        if (i >= G::NSFULL && !tail_on) continue;
-                                        const float4 ry = rays[sbase + 32 * i];
-                                        float s = ry.w * inv_d;
-                                        s = (s >= args.inv_range_max) ? s : CUDART_NAN_F;
-                                        bool ok;
-                                        float b = warp_sample<IDENT, FULLDIST, CHECKDEN, F16>(ry.x, ry.y, ry.z, s, args.views[v], fv, centre, ok);
-                                        b_s[sbase + 32 * i] = b;
-                                        all_ok = all_ok && ok;
+                                    for (int i0 = 0; i0 < NS; i0 += SBATCH) {
+                                        float au[SBATCH], av[SBATCH];
+                                        unsigned idx[SBATCH];
+                                        unsigned okm = 0u;
+                                        FootRaw<F16> raw[SBATCH];
+#pragma unroll
+                                        for (int jj = 0; jj < SBATCH; ++jj) {
+                                            au[jj] = 0.f; av[jj] = 0.f; idx[jj] = 0u;
+                                            const int i = i0 + jj;
+                                            if (i < NS) {
+                                                const float4 ry = rays[sbase + 32 * i];
+                                                float s = ry.w * inv_d;
+                                                s = (s >= args.inv_range_max) ? s : CUDART_NAN_F;
+                                                SampleAddr a = sample_addr<IDENT, FULLDIST, CHECKDEN>(ry.x, ry.y, ry.z, s, args.views[v]);
+                                                const bool on = a.ok && (i < G::NSFULL || tail_on); /* a pixel in this slot */
+                                                au[jj] = a.au; av[jj] = a.av;
+                                                idx[jj] = on ? a.idx : 0u;
+                                                okm |= on ? (1u << jj) : 0u;
+                                            }
+                                        }
+#pragma unroll
+                                        for (int jj = 0; jj < SBATCH; ++jj)
+                                            if (i0 + jj < NS) raw[jj] = foot_fetch<F16>(fv, idx[jj]);
+#pragma unroll
+                                        for (int jj = 0; jj < SBATCH; ++jj) {
+                                            const int i = i0 + jj;
+                                            if (i < NS) {
+                                                const bool ok = (okm >> jj) & 1u;
+                                                const float b = foot_lerp<F16>(raw[jj], au[jj], av[jj], ok, centre);
+                                                if (i < G::NSFULL || tail_on) {
+                                                    b_s[sbase + 32 * i] = b;
+                                                    all_ok = all_ok && ok;
+                                                }
+                                            }
+                                        }
                                     }
                                     all_ok = __all_sync(0xffffffffu, all_ok);
                                 }
