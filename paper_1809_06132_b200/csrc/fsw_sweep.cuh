@@ -68,12 +68,13 @@ struct Geo {
     static constexpr int HS = TX + 4;                  /* row stride of the row-sum planes, == 4 (mod 8) */
     static constexpr int PLANE = EHA * SB;
     static constexpr int HPLANE = EHA * HS;
-    static constexpr bool A_IN_REGS = WIN <= 9;        /* keep the a' operands of the horizontal item in registers */
+        static constexpr bool A_IN_REGS = WIN <= 9;               /* keep the a' operands of the horizontal item in registers */
     static_assert(EH <= EHA && TX % 32 == 0 && TX % RUN == 0 && NRUN == 8, "tile / thread mapping");
     static_assert(SB >= SBMIN && SB % 4 == 0 && HS % 8 == 4, "aligned strides");
     static_assert(R * NRUN <= 32, "one horizontal work item per lane");
     static constexpr size_t smem() {
-        return sizeof(float4) * PLANE + sizeof(float) * ((size_t)2 * PLANE + (size_t)4 * HPLANE);
+        return sizeof(float4) * PLANE + sizeof(float) * ((size_t)2 * PLANE + (size_t)4 * HPLANE) +
+               sizeof(float2) * TX * TY;
     }
 };
 
@@ -392,10 +393,9 @@ __global__ void __launch_bounds__(Geo<WIN>::NT, 1) sweep_kernel(const __grid_con
     constexpr int HW = G::HW, RPT = G::RPT, NS = G::NS, TX = G::TX, TY = G::TY, R = G::R;
     constexpr float NWIN = (float)(WIN * WIN);
     constexpr float INV_NWIN = 1.f / NWIN;
-#ifndef FSW_SBATCH
-#define FSW_SBATCH 4
-#endif
-    constexpr int SBATCH = FSW_SBATCH; /* samples in flight per lane */
+    /* samples in flight per lane: four with the 8-byte footprints of the specialised variant, two otherwise (the raw
+     * footprints of a batch stay in registers) */
+    constexpr int SBATCH = (IDENT && F16) ? 4 : 2;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     float4* rays = reinterpret_cast<float4*>(smem_raw);   /* [EHA][SB]: unit ray, .w = validity / incidence */
     float* a_s = reinterpret_cast<float*>(rays + G::PLANE); /* [EHA][SB]: centred reference intensities a' */
@@ -409,6 +409,8 @@ __global__ void __launch_bounds__(Geo<WIN>::NT, 1) sweep_kernel(const __grid_con
 
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     const int col = tid % TX, grp = tid / TX;
+    /* [TY][TX]: reference-side window statistics of every output: ((sum a')/N, sum a'^2 - (sum a')^2/N) */
+    float2* const a_stat = reinterpret_cast<float2*>(hs + 4 * G::HPLANE) + (grp * RPT) * TX + col;
     const int W = args.ref.W, H = args.ref.H;
     const int n_items = args.n_tiles * args.n_sets;
     const int n_views = NVT ? NVT : args.n_views;
@@ -451,9 +453,6 @@ __global__ void __launch_bounds__(Geo<WIN>::NT, 1) sweep_kernel(const __grid_con
         }
         bool tile_active = false;
         unsigned active_mask = 0; /* bit i: output i of this thread can have a finite cost */
-        float A1n[RPT], A2[RPT];  /* (sum a')/N and sum a'^2 - (sum a')^2/N of the output's window */
-#pragma unroll
-        for (int i = 0; i < RPT; ++i) { A1n[i] = 0.f; A2[i] = 0.f; }
         float centre = 0.f;
         float areg[G::NV4 * 4];   /* a' operands of this lane's horizontal work item */
 #pragma unroll
@@ -531,8 +530,8 @@ __global__ void __launch_bounds__(Geo<WIN>::NT, 1) sweep_kernel(const __grid_con
                     bool in_roi = ox >= args.roi_x0 && ox < args.roi_x1 && oy >= args.roi_y0 && oy < args.roi_y1;
                     bool act = in_roi && (sf[i] == NWIN); /* every window pixel inside the image and the FOV */
                     if (act) active_mask |= 1u << i;
-                    A1n[i] = sa[i] * INV_NWIN;
-                    A2[i] = fmaf(-A1n[i], sa[i], saa[i]);
+                    const float a1n = sa[i] * INV_NWIN;
+                    a_stat[i * TX] = make_float2(a1n, fmaf(-a1n, sa[i], saa[i]));
                 }
             }
             if (tid == 0) { s_mixed[0] = 0u; s_mixed[1] = 0u; s_mixed[2] = 0u; s_any[0] = 0u; s_any[1] = 0u; s_any[2] = 0u; }
@@ -678,9 +677,10 @@ __global__ void __launch_bounds__(Geo<WIN>::NT, 1) sweep_kernel(const __grid_con
                                 for (int i = 0; i < RPT; ++i) {
                                     bool okv = (active_mask >> i) & 1u;
                                     if (f_mixed) okv = okv && (sv[i] == NWIN);
-                                    float cov = fmaf(-A1n[i], sb[i], sab[i]);
+                                    const float2 A = a_stat[i * TX]; /* written by this thread */
+                                    float cov = fmaf(-A.x, sb[i], sab[i]);
                                     float vb = fmaf(-sb[i] * INV_NWIN, sb[i], sbb[i]);
-                                    float prod = fmaxf(A2[i] * vb, args.floor2);
+                                    float prod = fmaxf(A.y * vb, args.floor2);
                                     float z = cov * rsqrt_approx(prod);
                                     float cst = __saturatef(fmaf(-0.5f, z, 0.5f));
                                     acc[i] += okv ? cst : 0.f;
