@@ -29,6 +29,8 @@ import numpy as np  # noqa: E402
 FLOP_PER_EVAL = 70.0   # algorithmic FP32 work of one (pixel, plane, view) cost evaluation
 N_STAGED = 32          # distinct frame sets resident on the device (the C5 stream length)
 METRIC = "plane-sweep cost evals/sec (pixel x plane x view)"
+# dram__bytes_read.sum + dram__bytes_write.sum of one sweep launch, from the committed ncu capture (profiles/)
+NCU_DRAM_BYTES_PER_LAUNCH = {("C5", 8): 157.3e6}
 
 
 def parse_args():
@@ -40,7 +42,7 @@ def parse_args():
     ap.add_argument("--batch", type=int, default=8,
                     help="frame sets per sweep launch (fsw_compute_depth_batch); 1 = one launch per frame set")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--cpu-baseline-seconds", type=float, default=12.0)
+    ap.add_argument("--cpu-baseline-seconds", type=float, default=10.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
 
@@ -330,7 +332,12 @@ def run_ours(args, rank, local_rank, world):
                     "ms_per_step": ms_e2e / e2e_steps, "depth_maps_per_s": world * e2e_steps / (ms_e2e * 1e-3)},
             "gpu_launches": launches,
             "roofline": {"bound": "alu", "achieved": achieved, "peak": fp32_tflops, "unit": "TFLOP/s",
-                         "frac": achieved / fp32_tflops if fp32_tflops else None, "traffic": None,
+                         "frac": achieved / fp32_tflops if fp32_tflops else None,
+                         "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get((args.workload, B)),
+                         "traffic_source": "profiles/r1_launches_c5.md (ncu --set full, dram bytes read + written by "
+                                           "one sweep launch)" if (args.workload, B) in NCU_DRAM_BYTES_PER_LAUNCH else None,
+                         "ncu_issue_active_pct": 65.1 if (args.workload, B) in NCU_DRAM_BYTES_PER_LAUNCH else None,
+                         "frame_sets_per_launch": B, "evals_per_launch": evals_per_launch,
                          "kernel": "fsw::sweep_kernel<9,...>", "kernel_ms": sweep_ms_avg,
                          "flop_per_eval": FLOP_PER_EVAL,
                          "peak_source": "FFMA-chain kernel measured in this run (MEASURED_PEAKS.json has no FP32 figure); "
@@ -338,26 +345,28 @@ def run_ours(args, rank, local_rank, world):
         }
         line["depth_maps_per_s"] = world * args.steps / (ms_total * 1e-3)
         if not args.no_cpu_baseline:
-            line["cpu_baseline"] = cpu_baseline(cfg, host_frames[0], host_masks[0] if host_masks else None,
-                                                args.cpu_baseline_seconds)
+            line["cpu_baseline"] = cpu_baseline(cfg, host_frames, host_masks, args.cpu_baseline_seconds)
         print(json.dumps(line), flush=True)
     if dist is not None:
         dist.barrier()
         dist.destroy_process_group()
 
 
-def cpu_baseline(cfg, frame, mask, seconds):
-    """The oracle as it stands, timed on this box's host cores on a bounded sample of the workload."""
+def cpu_baseline(cfg, frames, masks, seconds):
+    """The oracle as it stands, timed on this box's host cores on a bounded sample of the workload: whole frame sets
+    of the stream (every plane and view), one after the other, until `seconds` of CPU work are done (at most 6)."""
     import oracle
     oracle.build()
     cores = oracle.num_threads()
-    planes_views = sum(f["n_planes"] for f in cfg["families"]) * (len(cfg["cams"]) - 1)
-    px = seconds * 1.2e6 * cores / planes_views
-    crop_h = int(min(640, max(64, (px * 0.75) ** 0.5))) // 4 * 4
-    crop_w = int(min(848, crop_h * 4 // 3)) // 4 * 4
-    dt, ne = oracle_sample(cfg, frame, mask, crop_w, crop_h)
-    return {"value": ne / dt, "unit": "evals/s", "cores": cores, "kind": "oracle", "seconds": dt,
-            "sample": "frame set 0, centred %dx%d crop (principal point shifted), all planes and views" % (crop_w, crop_h)}
+    W, H = cfg["cams"][0]["width"], cfg["cams"][0]["height"]
+    total_t, total_e, n = 0.0, 0, 0
+    while n < min(6, len(frames)) and total_t < seconds:
+        dt, ne = oracle_sample(cfg, frames[n], masks[n] if masks else None, W, H)
+        total_t += dt
+        total_e += ne
+        n += 1
+    return {"value": total_e / total_t, "unit": "evals/s", "cores": cores, "kind": "oracle", "seconds": total_t,
+            "sample": "frame sets 0..%d of the workload at full size (%dx%d), all planes and views" % (n - 1, W, H)}
 
 
 def main():
