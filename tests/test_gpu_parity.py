@@ -242,3 +242,25 @@ def test_batch_equals_single_calls():
     assert st["index_match_frac"] >= 0.999 and st["max_dc1"] <= 1e-4 and st["valid_mismatch_nonfragile"] == 0, st
     with pytest.raises(fsw.FswError):
         ctx.compute_depth_batch(planes, p, [], None)
+
+
+def test_bfloat16_and_float_footprints_agree_bitwise():
+    """8-bit views are staged as bfloat16 footprints (exact for integers up to 256), float views as float footprints:
+    the same integer-valued views given as uint8 and as float32 must produce bit-identical maps, and a call that
+    mixes both types (falls back to float footprints) as well."""
+    import torch
+    import paper_1809_06132_b200 as fsw
+    cfg = _small_rig(W=131, H=83, n_views=2, fov=170.0)
+    images = synth.render_frame(cfg, 0)
+    assert images[0].dtype == np.uint8
+    _, _, ctx = gpu_objects(cfg)
+    planes = fsw.PlaneSet(cfg["families"])
+    outs = []
+    # the reference image stays 8-bit (its type decides how the centring constant is rounded); only the views change
+    for kinds in (("u8", "u8", "u8"), ("u8", "f32", "f32"), ("u8", "f32", "u8")):
+        dev = [torch.from_numpy(im if k == "u8" else im.astype(np.float32)).cuda() for im, k in zip(images, kinds)]
+        outs.append(oracle.compare.to_numpy(ctx.compute_depth(planes, cfg["params"], dev)))
+    for o in outs[1:]:
+        for key in ("depth", "best_cost", "second_cost", "plane_index", "valid_reason"):
+            assert np.array_equal(outs[0][key], o[key], equal_nan=True), key
+    assert (outs[0]["plane_index"] >= 0).sum() > 1000
