@@ -84,6 +84,7 @@ def _load():
         L.orc_pixel_costs.argtypes = [cam, I, I, fam, I, prm, ctypes.POINTER(dp), I, I, dp]
         L.orc_wta.argtypes = [cam, fam, I, prm, dp, dp, dp, dp, dp, ip, dp, dp, bp]
         L.orc_filter_mask.argtypes = [I, I, prm, bp, bp, dp, dp, dp, bp, bp]
+        L.orc_filter_continuity.argtypes = [dp, I, I, I, D, D, bp, dp, bp]
         L.orc_downsample2.argtypes = [dp, I, I, dp]
         L.orc_camera_half.argtypes = [cam, cam]
         L.orc_camera_half.restype = None
@@ -271,6 +272,20 @@ def filter_mask(params, maps, mask=None):
                             _dp(maps["depth"]), _bp(reason), _bp(frag))
     maps["reason"], maps["valid"], maps["fragile_thr"] = reason, (reason == 0).astype(np.uint8), frag
     return maps
+
+
+def filter_continuity(depth, window=5, gamma=0.5, delta=0.3, mask=None):
+    """Local depth-continuity filter (third filter; reading Q25) followed by the mask.
+    depth: H x W, 0 = invalid.  -> (filtered depth float64, reason uint8)."""
+    a = np.ascontiguousarray(depth, dtype=np.float64)
+    H, W = a.shape
+    out = np.empty((H, W), dtype=np.float64)
+    reason = np.zeros((H, W), dtype=np.uint8)
+    m = None if mask is None else np.ascontiguousarray(mask, dtype=np.uint8)
+    rc = _load().orc_filter_continuity(_dp(a), W, H, int(window), float(gamma), float(delta), _bp(m), _dp(out), _bp(reason))
+    if rc != 0:
+        raise ValueError("filter_continuity: window must be odd and >= 3")
+    return out, reason
 
 
 def downsample2(img):

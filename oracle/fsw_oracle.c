@@ -491,6 +491,37 @@ int orc_filter_mask(int W, int H, const orc_params* prm, const uint8_t* mask, co
     return 0;
 }
 
+/* Third filter of PAPER.md:99, reading Q25: see fsw_oracle.h. */
+int orc_filter_continuity(const double* in, int W, int H, int window, double gamma, double delta,
+                          const uint8_t* mask, double* out, uint8_t* reason) {
+    if (window < 3 || window % 2 == 0) return -1;
+    const int hw = window / 2;
+    const double denom = (double)(window * window - 1);
+    for (int y = 0; y < H; ++y)
+        for (int x = 0; x < W; ++x) {
+            size_t i = (size_t)y * W + x;
+            double dc = in[i];
+            uint8_t why = ORC_OK;
+            if (!(dc > 0.0)) why = ORC_NO_PLANE;
+            else {
+                int consistent = 0;
+                for (int dy = -hw; dy <= hw; ++dy)
+                    for (int dx = -hw; dx <= hw; ++dx) {
+                        if (dx == 0 && dy == 0) continue;
+                        int xx = x + dx, yy = y + dy;
+                        if (xx < 0 || yy < 0 || xx >= W || yy >= H) continue; /* outside: not consistent */
+                        double dn = in[(size_t)yy * W + xx];
+                        if (dn > 0.0 && fabs(dn - dc) < gamma) ++consistent;
+                    }
+                if ((double)consistent / denom < delta) why = ORC_CONTINUITY;
+                else if (mask && mask[i]) why = ORC_MASKED;
+            }
+            reason[i] = why;
+            out[i] = why == ORC_OK ? dc : 0.0;
+        }
+    return 0;
+}
+
 /* ------------------------------------------------------------------------- */
 /* S10 multi-resolution (Q4, Q18, Q19)                         */
 /* ------------------------------------------------------------------------- */

@@ -41,6 +41,7 @@ extern "C" {
 #define ORC_COST_FILTER 2
 #define ORC_RATIO_FILTER 3
 #define ORC_MASKED 4
+#define ORC_CONTINUITY 5
 
 typedef struct {
     int32_t width, height;
@@ -125,6 +126,16 @@ int orc_filter_mask(int W, int H, const orc_params* prm, const uint8_t* mask /*n
                     const double* c1, const double* c2, double* depth, uint8_t* reason, uint8_t* fragile);
 
 /* S10(a): 2x2 box downsample of an image and of a camera (f/2, c' = (c-0.5)/2) */
+/* Local depth-continuity filter, the third filter of PAPER.md:99 ("we compare its depth value against the depths of its
+ * neighboring pixels in a local window ... smaller than a threshold gamma ... ratio of the consistent pixels ...
+ * smaller than delta"; gamma = 0.5 m, delta = 0.3).  Reading Q25: window x window neighbourhood without
+ * the centre; a neighbour is consistent iff it is valid (depth > 0), inside the image and |d_n - d_c| < gamma; the
+ * centre is invalidated iff consistent / (window^2 - 1) < delta (exactly delta is kept).  Reads `in` only (never a
+ * partially filtered state), then applies the mask (nullable).  out: depth (0 = invalid), reason: 0 kept,
+ * ORC_NO_PLANE where the input was invalid, ORC_CONTINUITY, ORC_MASKED. */
+int orc_filter_continuity(const double* in, int W, int H, int window, double gamma, double delta,
+                          const uint8_t* mask /*nullable*/, double* out, uint8_t* reason);
+
 int orc_downsample2(const double* img, int W, int H, double* out);
 void orc_camera_half(const orc_camera* c, orc_camera* out);
 
