@@ -80,6 +80,7 @@ extern "C" {
 #define FSW_REASON_COST_FILTER 2
 #define FSW_REASON_RATIO_FILTER 3
 #define FSW_REASON_MASKED 4
+#define FSW_REASON_CONTINUITY 5   /* fsw_filter_continuity: too few consistent neighbours */
 
 /* bit set in plane_index where the full-resolution crop pass supplied the value (multi-resolution call) */
 #define FSW_INDEX_FROM_CROP (1 << 14)
@@ -256,6 +257,26 @@ int32_t fsw_context_set_timing(fsw_context* ctx, int32_t on);
 
 /* Counters of the most recent compute call on this context.  Synchronizes the stream that call used. */
 int32_t fsw_get_last_counters(fsw_context* ctx, fsw_counters* out);
+
+/* ---- local depth-continuity filter ------------------------------------------ */
+/* The third filter of PAPER.md:99 ("we compare its depth value against the depths of its neighboring pixels in a local
+ * window. If the difference is smaller than a threshold gamma, we will consider the neighboring pixels to be consistent
+ * with the central pixel. If the ratio of the consistent pixels in the local window is smaller than delta, we will
+ * consider the center pixel to have inaccurate depth"; gamma = 0.5 m, delta = 0.3), followed by the mask.
+ * Reading Q25: window x window neighbourhood (odd, 3..FSW_MAX_WINDOW; SPEC.md proposes 5) without the
+ * centre; a neighbour is consistent iff it is valid (depth > 0), inside the image and |d_n - d_c| < gamma (compared in
+ * double precision); the centre is invalidated iff consistent / (window^2 - 1) < delta.  Only depth_in is read (never a
+ * partially filtered state), so depth_out must not overlap depth_in.
+ * depth_in / depth_out: device, float32, reference-camera size of the context's rig, pitches in BYTES, 0.0f = invalid.
+ * Call fsw_compute_depth* WITHOUT a mask and pass the mask here (nullable): the mask comes after the filters.
+ * reason_out (device, nullable, uint8): FSW_REASON_OK, FSW_REASON_NO_PLANE where depth_in was invalid,
+ * FSW_REASON_CONTINUITY, FSW_REASON_MASKED.  Asynchronous on cuda_stream.
+ * Errors: FSW_E_INVALID_ARG (null pointers, even / out-of-range window, gamma <= 0, delta outside [0,1], pitches too
+ * small, overlapping depth buffers), FSW_E_CUDA. */
+int32_t fsw_filter_continuity(fsw_context* ctx, const float* depth_in, size_t depth_in_pitch, int32_t window,
+                              float gamma, float delta, const uint8_t* mask, size_t mask_pitch,
+                              float* depth_out, size_t depth_out_pitch, uint8_t* reason_out, size_t reason_pitch,
+                              void* cuda_stream);
 
 /* ---- measurement helper ---------------------------------------------------- */
 /* Runs a dependent-FFMA-chain kernel on `cuda_stream` and reports the FP32 throughput it reached (TFLOP/s, counting

@@ -28,7 +28,7 @@ EXPORTS = (
     "fsw_planeset_table", "fsw_context_create", "fsw_context_destroy", "fsw_compute_depth",
     "fsw_compute_depth_multires", "fsw_compute_depth_host", "fsw_compute_depth_multires_host",
     "fsw_compute_depth_batch", "fsw_compute_depth_batch_host",
-    "fsw_context_set_timing", "fsw_get_last_counters", "fsw_measure_fp32_peak",
+    "fsw_context_set_timing", "fsw_get_last_counters", "fsw_measure_fp32_peak", "fsw_filter_continuity",
 )
 
 
@@ -404,6 +404,25 @@ class Context:
                   CRect(*[int(x) for x in crop]), arr, mptr, mpitch, ctypes.byref(cout), stream))
         out["_keep"] = (keep, mkeep)
         return out
+
+    def filter_continuity(self, depth, window=5, gamma=0.5, delta=0.3, mask=None, want_reason=True):
+        """fsw_filter_continuity: the local depth-continuity filter of PAPER.md:99 + mask on a device depth map.
+        Returns dict(depth=..., valid_reason=...) of new device tensors."""
+        torch = _torch()
+        W, H = self.rig.sizes[self.rig.ref_index]
+        assert depth.is_cuda and depth.dtype == torch.float32 and tuple(depth.shape) == (H, W) and depth.stride(1) == 1
+        out = torch.empty((H, W), dtype=torch.float32, device=depth.device)
+        reason = torch.empty((H, W), dtype=torch.uint8, device=depth.device) if want_reason else None
+        mptr, mpitch, mkeep = self._mask(mask, False)
+        stream = torch.cuda.current_stream(self.device).cuda_stream
+        fn = load_library().fsw_filter_continuity
+        fn.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_size_t, ctypes.c_int32, ctypes.c_float, ctypes.c_float,
+                       ctypes.c_void_p, ctypes.c_size_t, ctypes.c_void_p, ctypes.c_size_t, ctypes.c_void_p,
+                       ctypes.c_size_t, ctypes.c_void_p]
+        _check(fn(self.handle, depth.data_ptr(), depth.stride(0) * 4, int(window), float(gamma), float(delta),
+                  mptr, mpitch, out.data_ptr(), out.stride(0) * 4,
+                  None if reason is None else reason.data_ptr(), 0 if reason is None else reason.stride(0), stream))
+        return dict(depth=out, valid_reason=reason, _keep=(depth, mkeep))
 
     def last_counters(self):
         c = CCounters()

@@ -905,6 +905,36 @@ int32_t fsw_compute_depth_multires_host(fsw_context* ctx, const fsw_planeset* pl
     return run_host(ctx, true, planes_low, planes_crop, params_low, params_crop, crop, 1, images, mask ? masks : nullptr, mask_pitch, out, cuda_stream);
 }
 
+int32_t fsw_filter_continuity(fsw_context* ctx, const float* depth_in, size_t depth_in_pitch, int32_t window,
+                              float gamma, float delta, const uint8_t* mask, size_t mask_pitch,
+                              float* depth_out, size_t depth_out_pitch, uint8_t* reason_out, size_t reason_pitch,
+                              void* cuda_stream) {
+    if (!ctx || !depth_in || !depth_out) return fail(FSW_E_INVALID_ARG, "fsw_filter_continuity: null context or depth buffer");
+    if (window < 3 || window > FSW_MAX_WINDOW || window % 2 == 0)
+        return fail(FSW_E_INVALID_ARG, "fsw_filter_continuity: window=%d must be odd and in 3..%d", window, FSW_MAX_WINDOW);
+    if (!(gamma > 0.f) || !(delta >= 0.f && delta <= 1.f))
+        return fail(FSW_E_INVALID_ARG, "fsw_filter_continuity: gamma=%g must be > 0 and delta=%g in [0,1]", (double)gamma, (double)delta);
+    const fsw_camera& ref = ctx->rig.cams[ctx->rig.ref_index];
+    const int W = ref.width, H = ref.height;
+    if (depth_in_pitch < (size_t)W * 4 || depth_out_pitch < (size_t)W * 4 || (mask && mask_pitch < (size_t)W) ||
+        (reason_out && reason_pitch < (size_t)W))
+        return fail(FSW_E_INVALID_ARG, "fsw_filter_continuity: a pitch is smaller than one row of %d pixels", W);
+    const char* i0 = (const char*)depth_in; const char* i1 = i0 + depth_in_pitch * (size_t)H;
+    const char* o0 = (const char*)depth_out; const char* o1 = o0 + depth_out_pitch * (size_t)H;
+    if (i0 < o1 && o0 < i1) return fail(FSW_E_INVALID_ARG, "fsw_filter_continuity: depth_out overlaps depth_in");
+    DeviceGuard g;
+    FSW_CUDA(g.enter(ctx->device));
+    FswContinuityArgs a;
+    a.in = depth_in; a.in_pitch = (int64_t)depth_in_pitch;
+    a.out = depth_out; a.out_pitch = (int64_t)depth_out_pitch;
+    a.mask = mask; a.mask_pitch = (int64_t)mask_pitch;
+    a.reason = reason_out; a.reason_pitch = (int64_t)reason_pitch;
+    a.W = W; a.H = H; a.window = window;
+    a.gamma = (double)gamma; a.delta = (double)delta;
+    FSW_CUDA(fsw_launch_continuity(a, (cudaStream_t)cuda_stream));
+    return FSW_OK;
+}
+
 int32_t fsw_context_set_timing(fsw_context* ctx, int32_t on) {
     if (!ctx) return fail(FSW_E_INVALID_ARG, "fsw_context_set_timing: null context");
     DeviceGuard g;

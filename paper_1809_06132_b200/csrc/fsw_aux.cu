@@ -75,6 +75,44 @@ __global__ void __launch_bounds__(256) downsample_kernel(const __grid_constant__
     a.dst[cam][(int64_t)y * W2 + x] = 0.25f * s;
 }
 
+/* Local depth-continuity filter (third filter; reading Q25 of DESIGN.md) + mask.  One thread per pixel,
+ * a 32 x 16 tile plus its halo staged in shared memory (0 = invalid, also outside the image); the comparisons run in
+ * double precision so that the result is a function of the float32 input map alone. */
+constexpr int CT_X = 32, CT_Y = 16, CT_HALO = FSW_MAX_WINDOW / 2;
+__global__ void __launch_bounds__(CT_X * CT_Y) continuity_kernel(const __grid_constant__ FswContinuityArgs a) {
+    __shared__ float tile[CT_Y + 2 * CT_HALO][CT_X + 2 * CT_HALO + 1];
+    const int hw = a.window / 2;
+    const int x0 = blockIdx.x * CT_X - hw, y0 = blockIdx.y * CT_Y - hw;
+    const int tw = CT_X + 2 * hw, th = CT_Y + 2 * hw;
+    for (int i = threadIdx.y * CT_X + threadIdx.x; i < tw * th; i += CT_X * CT_Y) {
+        const int ty = i / tw, tx = i - ty * tw;
+        const int x = x0 + tx, y = y0 + ty;
+        float d = 0.f;
+        if (x >= 0 && y >= 0 && x < a.W && y < a.H)
+            d = __ldg(reinterpret_cast<const float*>(reinterpret_cast<const char*>(a.in) + (int64_t)y * a.in_pitch) + x);
+        tile[ty][tx] = d;
+    }
+    __syncthreads();
+    const int x = blockIdx.x * CT_X + threadIdx.x, y = blockIdx.y * CT_Y + threadIdx.y;
+    if (x >= a.W || y >= a.H) return;
+    const float dcf = tile[threadIdx.y + hw][threadIdx.x + hw];
+    int reason = FSW_REASON_OK;
+    if (!(dcf > 0.f)) reason = FSW_REASON_NO_PLANE;
+    else {
+        const double dc = (double)dcf;
+        int consistent = 0;
+        for (int dy = 0; dy < a.window; ++dy)
+            for (int dx = 0; dx < a.window; ++dx) {
+                const float dn = tile[threadIdx.y + dy][threadIdx.x + dx];
+                if ((dx != hw || dy != hw) && dn > 0.f && fabs((double)dn - dc) < a.gamma) ++consistent;
+            }
+        if ((double)consistent / (double)(a.window * a.window - 1) < a.delta) reason = FSW_REASON_CONTINUITY;
+        else if (a.mask != nullptr && a.mask[(int64_t)y * a.mask_pitch + x]) reason = FSW_REASON_MASKED;
+    }
+    *(reinterpret_cast<float*>(reinterpret_cast<char*>(a.out) + (int64_t)y * a.out_pitch) + x) = reason == FSW_REASON_OK ? dcf : 0.f;
+    if (a.reason != nullptr) a.reason[(int64_t)y * a.reason_pitch + x] = (uint8_t)reason;
+}
+
 /* 8 independent FFMA chains per thread; 2 flop per FFMA */
 __global__ void __launch_bounds__(256) ffma_peak_kernel(float* sink, int iters) {
     float x0 = threadIdx.x * 1e-3f, x1 = x0 + 1.f, x2 = x0 + 2.f, x3 = x0 + 3.f;
@@ -107,6 +145,12 @@ cudaError_t fsw_launch_downsample(const FswDownArgs& args, cudaStream_t stream) 
     }
     dim3 grid((maxW + 255) / 256, maxH, args.n);
     downsample_kernel<<<grid, 256, 0, stream>>>(args);
+    return cudaGetLastError();
+}
+
+cudaError_t fsw_launch_continuity(const FswContinuityArgs& args, cudaStream_t stream) {
+    dim3 grid((args.W + CT_X - 1) / CT_X, (args.H + CT_Y - 1) / CT_Y, 1);
+    continuity_kernel<<<grid, dim3(CT_X, CT_Y, 1), 0, stream>>>(args);
     return cudaGetLastError();
 }
 

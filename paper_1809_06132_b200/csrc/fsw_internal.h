@@ -145,6 +145,16 @@ struct FswDownArgs {
 };
 cudaError_t fsw_launch_downsample(const FswDownArgs& args, cudaStream_t stream);
 
+struct FswContinuityArgs {
+    const float* in; int64_t in_pitch;     /* bytes */
+    float* out; int64_t out_pitch;
+    const uint8_t* mask; int64_t mask_pitch;
+    uint8_t* reason; int64_t reason_pitch;
+    int32_t W, H, window;
+    double gamma, delta;
+};
+cudaError_t fsw_launch_continuity(const FswContinuityArgs& args, cudaStream_t stream);
+
 cudaError_t fsw_launch_ffma_peak(float* sink, int blocks, int iters, cudaStream_t stream);
 
 #endif

@@ -34,7 +34,6 @@
 #define FSW_SWEEP_CUH
 
 #include <math_constants.h>
-#include <cstdio>
 
 #include "fsw_internal.h"
 
@@ -68,7 +67,7 @@ struct Geo {
     static constexpr int HS = TX + 4;                  /* row stride of the row-sum planes, == 4 (mod 8) */
     static constexpr int PLANE = EHA * SB;
     static constexpr int HPLANE = EHA * HS;
-        static constexpr bool A_IN_REGS = WIN <= 9;               /* keep the a' operands of the horizontal item in registers */
+    static constexpr bool A_IN_REGS = WIN <= 9;        /* keep the a' operands of the horizontal item in registers */
     static_assert(EH <= EHA && TX % 32 == 0 && TX % RUN == 0 && NRUN == 8, "tile / thread mapping");
     static_assert(SB >= SBMIN && SB % 4 == 0 && HS % 8 == 4, "aligned strides");
     static_assert(R * NRUN <= 32, "one horizontal work item per lane");
@@ -202,12 +201,6 @@ __device__ __forceinline__ SampleAddr sample_addr(float rx, float ry, float rz, 
     a.au = u - (tu - 12582912.f);
     a.av = v - (tv - 12582912.f);
     a.idx = ok ? iy * (unsigned)k.cam.W + ix : 0u; /* invalid samples fetch footprint 0 instead of branching */
-#ifdef FSW_DEBUG_CLAMP
-    a.idx = min(a.idx, (unsigned)(k.cam.W * k.cam.H - 1));
-#endif
-#ifdef FSW_DEBUG_BOUNDS
-    if (a.idx >= (unsigned)(k.cam.W * k.cam.H)) { printf("bad idx %u ix %u iy %u ok %d W %d H %d\n", a.idx, ix, iy, (int)ok, k.cam.W, k.cam.H); a.idx = 0; }
-#endif
     a.ok = ok;
     return a;
 }
@@ -589,9 +582,6 @@ __global__ void __launch_bounds__(Geo<WIN>::NT, 1) sweep_kernel(const __grid_con
                                 bool all_ok = true;
                                 if (rows_on) {
                                     const void* fv = s_set.foot[v];
-#ifdef FSW_DEBUG_BOUNDS
-                                    if (fv == nullptr || v >= args.n_views) printf("bad foot v %d %p\n", v, fv);
-#endif
                                     /* batches of SBATCH samples: all addresses, then all fetches, then the lerps */
 #pragma unroll
                                     for (int i0 = 0; i0 < NS; i0 += SBATCH) {

@@ -264,3 +264,51 @@ def test_bfloat16_and_float_footprints_agree_bitwise():
         for key in ("depth", "best_cost", "second_cost", "plane_index", "valid_reason"):
             assert np.array_equal(outs[0][key], o[key], equal_nan=True), key
     assert (outs[0]["plane_index"] >= 0).sum() > 1000
+
+
+@pytest.mark.parametrize("idx,window,gamma,delta", [(2, 5, 0.5, 0.3), (3, 5, 0.5, 0.3), (2, 9, 0.2, 0.5), (1, 3, 2.0, 0.25)])
+def test_continuity_filter_bit_exact_against_oracle(idx, window, gamma, delta):
+    """fsw_filter_continuity (third filter + mask) on the depth map the sweep produced: validity, reasons
+    and surviving depths must equal the oracle's filter on the same float32 map bit for bit (integer / comparison
+    work: both sides compare in double precision)."""
+    import torch
+    import paper_1809_06132_b200 as fsw
+    cfg = synth.make_config(idx)
+    images = synth.render_frame(cfg, 0)
+    W, H = cfg["cams"][0]["width"], cfg["cams"][0]["height"]
+    _, _, ctx = gpu_objects(cfg)
+    planes = fsw.PlaneSet(cfg["families"])
+    p = dict(cfg["params"], filters=3 if idx > 1 else 0, alpha_upper=0.3, alpha_lower=0.3, beta=1.1, horizon_row=H // 2)
+    dev = [torch.from_numpy(np.ascontiguousarray(im)).cuda() for im in images]
+    swept = ctx.compute_depth(planes, p, dev)          # no mask here: the mask comes after the filters
+    mask = synth.make_mask(W, H, 77, n_rects=3)
+    if idx == 1:  # the generator's rectangles are larger than this 64 x 48 image
+        mask = np.zeros((H, W), np.uint8)
+        mask[10:20, 30:50] = 1
+    out = ctx.filter_continuity(swept["depth"], window, gamma, delta, torch.from_numpy(mask).cuda())
+    torch.cuda.synchronize()
+    d_in = swept["depth"].cpu().numpy()
+    ref_d, ref_r = oracle.filter_continuity(d_in, window, gamma, delta, mask)
+    assert np.array_equal(out["valid_reason"].cpu().numpy(), ref_r)
+    assert np.array_equal(out["depth"].cpu().numpy().astype(np.float64), ref_d)
+    n_in, n_out = int((d_in > 0).sum()), int((ref_d > 0).sum())
+    assert 0 < n_out <= n_in
+    if idx > 1:  # the scenes with depth edges: every verdict occurs
+        assert n_out < n_in and (ref_r == 5).sum() > 0 and (ref_r == 4).sum() > 0
+    # without mask and reason map; pitched input view
+    out2 = ctx.filter_continuity(swept["depth"], window, gamma, delta, None, want_reason=False)
+    ref2, _ = oracle.filter_continuity(d_in, window, gamma, delta)
+    assert np.array_equal(out2["depth"].cpu().numpy().astype(np.float64), ref2)
+
+
+def test_continuity_filter_argument_errors():
+    import torch
+    import paper_1809_06132_b200 as fsw
+    cfg = _small_rig(W=64, H=48)
+    _, _, ctx = gpu_objects(cfg)
+    d = torch.ones((48, 64), dtype=torch.float32, device="cuda")
+    for kw in (dict(window=4), dict(window=17), dict(gamma=0.0), dict(delta=1.5)):
+        with pytest.raises(fsw.FswError):
+            ctx.filter_continuity(d, **kw)
+    out = ctx.filter_continuity(d)   # constant map: unchanged (SPEC.md:284)
+    assert torch.equal(out["depth"], d) and int(out["valid_reason"].sum()) == 0
