@@ -38,7 +38,7 @@ def parse_args():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=128)
     ap.add_argument("--warmup", type=int, default=8)
-    ap.add_argument("--workload", default="C5", choices=["C5", "C3"])
+    ap.add_argument("--workload", default="C5", choices=["C5", "C3", "P"])
     ap.add_argument("--batch", type=int, default=8,
                     help="frame sets per sweep launch (fsw_compute_depth_batch); 1 = one launch per frame set")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
@@ -49,13 +49,16 @@ def parse_args():
 
 def workload_config(name):
     import synth
-    cfg = synth.make_config(5 if name == "C5" else 3)
+    cfg = synth.make_config({"C5": 5, "C3": 3, "P": 6}[name])
     if name == "C3":  # the C3 scene, but as a stream of N_STAGED frame sets like C5 so that inputs exceed L2
         cfg = dict(cfg, n_frames=N_STAGED, step_m=0.5, mask_seed=None)
     return cfg
 
 
 def workload_label(name):
+    if name == "P":
+        return ("paper workload shape (PAPER.md:224,249; SURVEY 8(f) 2): 5 fisheye cams (4 matching views, rotated) "
+                "1024x544 u8, 64 fronto + 30 ground planes, 9x9 ZNCC, filters")
     return ("BASELINE.json configs[4]: 32-frame stream, 3 fisheye cams 1280x1024 u8, 192 fronto + 64 ground planes, "
             "9x9 ZNCC, filters + masks" if name == "C5" else
             "BASELINE.json configs[2]: 3 fisheye cams 1280x1024 u8, 96 fronto + 32 ground planes, 9x9 ZNCC, filters")
@@ -158,7 +161,7 @@ def run_reference(args, rank):
         f = s % N_STAGED
         if f not in frames:
             frames[f] = synth.render_frame(cfg, f)
-        mask = None if cfg.get("mask_seed") is None else synth.make_mask(1280, 1024, cfg["mask_seed"] + f)
+        mask = None if cfg.get("mask_seed") is None else synth.make_mask(cfg["cams"][0]["width"], cfg["cams"][0]["height"], cfg["mask_seed"] + f)
         dt, ne = oracle_sample(cfg, frames[f], mask, crop_w, crop_h)
         if s >= args.warmup:
             times.append(dt)

@@ -246,8 +246,24 @@ def _street_rig():
     return [camera(**kw), camera(centre=(-0.5, 0, 0), **kw), camera(centre=(0.5, 0, 0), **kw)]
 
 
+def _paper_rig():
+    """The shape of the paper's own workload: five fisheye cameras of 1024 x 544, the reference
+    in the middle and four matching views with rotated optical axes (values are this generator's, not the paper's:
+    its calibration is not published)."""
+    kw = dict(width=1024, height=544, fx=285.0, fy=285.0, cx=512.0, cy=272.0, xi=1.0, k1=-0.05, fov_max_deg=185.0)
+    return [camera(**kw), camera(centre=(-0.6, 0.0, 0.0), yaw_deg=-12.0, **kw), camera(centre=(0.6, 0.0, 0.0), yaw_deg=12.0, **kw),
+            camera(centre=(-0.25, -0.3, 0.1), yaw_deg=-4.0, **kw), camera(centre=(0.25, -0.3, 0.1), yaw_deg=4.0, **kw)]
+
+
 def make_config(index: int) -> dict:
-    """index = 1..5 for C1..C5 (BASELINE.json configs[index-1])."""
+    """index = 1..5 for C1..C5 (BASELINE.json configs[index-1]); 6 = the paper's own workload shape:
+    5 cameras (4 matching views) of 1024 x 544, 64 fronto-parallel + 30 ground-parallel planes, 9 x 9 ZNCC, as a
+    stream of 32 frame sets."""
+    if index == 6:
+        return dict(name="P", dtype="u8", ref_index=0, cams=_paper_rig(), n_frames=32, step_m=0.5, mask_seed=None,
+                    families=[family((0, 0, 1), 64, 0.5, 50.0, "inverse"), family((0, 1, 0), 30, 1.1, 2.1, "linear")],
+                    params=params(9, VAR_FLOOR_U8, 100.0, 0.05, 0.3, 272, 1.2, filters=FILTER_COST | FILTER_RATIO),
+                    scene=scene_street(seed=3))
     if index == 1:
         kw = dict(width=64, height=48, fx=30.0, fy=30.0, cx=32.0, cy=24.0, xi=0.9, fov_max_deg=200.0)
         return dict(name="C1", dtype="u8", ref_index=0,
@@ -285,7 +301,7 @@ def make_config(index: int) -> dict:
                               family((0, 1, 0), 64, 1.1, 2.1, "linear")],
                     params=params(9, VAR_FLOOR_U8, 100.0, 0.05, 0.3, 512, 1.2, filters=fil),
                     scene=scene_street(seed=3))
-    raise ValueError("config index must be 1..5")
+    raise ValueError("config index must be 1..6")
 
 
 @lru_cache(maxsize=8)

@@ -43,6 +43,16 @@ def test_config_single_resolution(idx):
     assert counters["n_launches"] >= 1
 
 
+def test_paper_workload_shape_four_rotated_views():
+    """the paper's own workload shape (5 cameras = 4 rotated matching views, 1024x544, 64 + 30 planes,
+    9x9): the run-time view loop of the generic kernel variant at full size."""
+    cfg = synth.make_config(6)
+    images = synth.render_frame(cfg, 3)
+    _, _, stats, counters = run_single(cfg, images)
+    assert_gates(stats)
+    assert stats["n_oracle_valid"] > 50000 and counters["n_eval"] > 10_000_000
+
+
 @pytest.mark.parametrize("idx", [1, 2])
 def test_config_with_filters(idx):
     """C1 / C2 name no filters; SURVEY 8(d) asks for both the raw-valid set and alpha = 0.3/0.3, beta = 1.2."""
