@@ -373,6 +373,58 @@ __device__ __forceinline__ void h_item(int lane, int& row, int& run) {
     }
 }
 
+/* S2-S4 for the R halo rows of one warp and one (plane, view): samples into the warp's rows of b_s (NaN = invalid).
+ * Returns (warp-uniform) whether every sample of the rows is valid. */
+template <class G, bool IDENT, bool FULLDIST, bool CHECKDEN, bool F16>
+__device__ __forceinline__ bool sample_rows(const float4* __restrict__ rays, float* __restrict__ b_s, int sbase, bool tail_on,
+                                            float inv_d, float s_min, const FswDevView& view,
+                                            const void* __restrict__ fv, float centre) {
+    constexpr int NS = G::NS;
+    /* samples in flight per lane: four with the 8-byte footprints of the specialised variant, two otherwise (the raw
+     * footprints of a batch stay in registers) */
+    constexpr int SBATCH = (IDENT && F16) ? 4 : 2;
+    bool all_ok = true;
+    /* batches of SBATCH samples: all addresses, then all fetches, then the lerps */
+#pragma unroll
+    for (int i0 = 0; i0 < NS; i0 += SBATCH) {
+        float au[SBATCH], av[SBATCH];
+        unsigned idx[SBATCH];
+        unsigned okm = 0u;
+        FootRaw<F16> raw[SBATCH];
+#pragma unroll
+        for (int jj = 0; jj < SBATCH; ++jj) {
+            au[jj] = 0.f; av[jj] = 0.f; idx[jj] = 0u;
+            const int i = i0 + jj;
+            if (i < NS) {
+                const float4 ry = rays[sbase + 32 * i];
+                float s = ry.w * inv_d;
+                s = (s >= s_min) ? s : CUDART_NAN_F;
+                SampleAddr a = sample_addr<IDENT, FULLDIST, CHECKDEN>(ry.x, ry.y, ry.z, s, view);
+                const bool on = a.ok && (i < G::NSFULL || tail_on); /* a pixel in this slot */
+                au[jj] = a.au; av[jj] = a.av;
+                idx[jj] = on ? a.idx : 0u;
+                okm |= on ? (1u << jj) : 0u;
+            }
+        }
+#pragma unroll
+        for (int jj = 0; jj < SBATCH; ++jj)
+            if (i0 + jj < NS) raw[jj] = foot_fetch<F16>(fv, idx[jj]);
+#pragma unroll
+        for (int jj = 0; jj < SBATCH; ++jj) {
+            const int i = i0 + jj;
+            if (i < NS) {
+                const bool ok = (okm >> jj) & 1u;
+                const float b = foot_lerp<F16>(raw[jj], au[jj], av[jj], ok, centre);
+                if (i < G::NSFULL || tail_on) {
+                    b_s[sbase + 32 * i] = b;
+                    all_ok = all_ok && ok;
+                }
+            }
+        }
+    }
+    return __all_sync(0xffffffffu, all_ok);
+}
+
 /* the fields of a frame set the sweep loop touches, staged in shared memory once per tile */
 struct SetHot {
     const void* foot[FSW_MAX_VIEWS];
@@ -386,9 +438,6 @@ __global__ void __launch_bounds__(Geo<WIN>::NT, 1) sweep_kernel(const __grid_con
     constexpr int HW = G::HW, RPT = G::RPT, NS = G::NS, TX = G::TX, TY = G::TY, R = G::R;
     constexpr float NWIN = (float)(WIN * WIN);
     constexpr float INV_NWIN = 1.f / NWIN;
-    /* samples in flight per lane: four with the 8-byte footprints of the specialised variant, two otherwise (the raw
-     * footprints of a batch stay in registers) */
-    constexpr int SBATCH = (IDENT && F16) ? 4 : 2;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     float4* rays = reinterpret_cast<float4*>(smem_raw);   /* [EHA][SB]: unit ray, .w = validity / incidence */
     float* a_s = reinterpret_cast<float*>(rays + G::PLANE); /* [EHA][SB]: centred reference intensities a' */
@@ -582,45 +631,8 @@ __global__ void __launch_bounds__(Geo<WIN>::NT, 1) sweep_kernel(const __grid_con
                                 bool all_ok = true;
                                 if (rows_on) {
                                     const void* fv = s_set.foot[v];
-                                    /* batches of SBATCH samples: all addresses, then all fetches, then the lerps */
-#pragma unroll
-                                    for (int i0 = 0; i0 < NS; i0 += SBATCH) {
-                                        float au[SBATCH], av[SBATCH];
-                                        unsigned idx[SBATCH];
-                                        unsigned okm = 0u;
-                                        FootRaw<F16> raw[SBATCH];
-#pragma unroll
-                                        for (int jj = 0; jj < SBATCH; ++jj) {
-                                            au[jj] = 0.f; av[jj] = 0.f; idx[jj] = 0u;
-                                            const int i = i0 + jj;
-                                            if (i < NS) {
-                                                const float4 ry = rays[sbase + 32 * i];
-                                                float s = ry.w * inv_d;
-                                                s = (s >= args.inv_range_max) ? s : CUDART_NAN_F;
-                                                SampleAddr a = sample_addr<IDENT, FULLDIST, CHECKDEN>(ry.x, ry.y, ry.z, s, args.views[v]);
-                                                const bool on = a.ok && (i < G::NSFULL || tail_on); /* a pixel in this slot */
-                                                au[jj] = a.au; av[jj] = a.av;
-                                                idx[jj] = on ? a.idx : 0u;
-                                                okm |= on ? (1u << jj) : 0u;
-                                            }
-                                        }
-#pragma unroll
-                                        for (int jj = 0; jj < SBATCH; ++jj)
-                                            if (i0 + jj < NS) raw[jj] = foot_fetch<F16>(fv, idx[jj]);
-#pragma unroll
-                                        for (int jj = 0; jj < SBATCH; ++jj) {
-                                            const int i = i0 + jj;
-                                            if (i < NS) {
-                                                const bool ok = (okm >> jj) & 1u;
-                                                const float b = foot_lerp<F16>(raw[jj], au[jj], av[jj], ok, centre);
-                                                if (i < G::NSFULL || tail_on) {
-                                                    b_s[sbase + 32 * i] = b;
-                                                    all_ok = all_ok && ok;
-                                                }
-                                            }
-                                        }
-                                    }
-                                    all_ok = __all_sync(0xffffffffu, all_ok);
+                                    all_ok = sample_rows<G, IDENT, FULLDIST, CHECKDEN, F16>(rays, b_s, sbase, tail_on, inv_d,
+                                        args.inv_range_max, args.views[v], fv, centre);
                                 }
                                 __syncwarp();
                                 /* ---- S5: horizontal box sums of the same rows --------------------------------- */
