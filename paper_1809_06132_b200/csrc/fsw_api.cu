@@ -340,13 +340,14 @@ FswSweepGeometry window_geometry(int w, int n_views) {
 
 /* picks the kernel variant the views allow (see fsw_sweep.cuh) */
 int pick_variant(const FswSweepArgs& a, int foot_f16) {
-    bool fast = true;
+    bool ident = true, simple = true;
     for (int v = 0; v < a.n_views; ++v) {
-        fast = fast && a.views[v].ident_R;
-        fast = fast && a.views[v].cam.dist_mode != FSW_DIST_FULL;
-        fast = fast && (a.views[v].cam.cos_fov_xi >= 1e-3f); /* lets the kernel drop the denominator test */
+        ident = ident && a.views[v].ident_R;
+        simple = simple && a.views[v].cam.dist_mode != FSW_DIST_FULL;
+        simple = simple && (a.views[v].cam.cos_fov_xi >= 1e-3f); /* lets the kernel drop the denominator test */
     }
-    return (fast ? 1 : 0) | (foot_f16 ? 2 : 0);
+    const int mode = !simple ? 0 : (ident ? 1 : 2);
+    return mode + (foot_f16 ? 3 : 0);
 }
 
 /* Scheduling order of the tiles (S0): nearest to the principal point first, lower image half before the upper

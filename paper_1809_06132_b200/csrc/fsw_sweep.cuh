@@ -382,7 +382,7 @@ __device__ __forceinline__ bool sample_rows(const float4* __restrict__ rays, flo
     constexpr int NS = G::NS;
     /* samples in flight per lane: four with the 8-byte footprints of the specialised variant, two otherwise (the raw
      * footprints of a batch stay in registers) */
-    constexpr int SBATCH = (IDENT && F16) ? 4 : 2;
+    constexpr int SBATCH = (!FULLDIST && F16) ? 4 : 2;
     bool all_ok = true;
     /* batches of SBATCH samples: all addresses, then all fetches, then the lerps */
 #pragma unroll
@@ -804,24 +804,29 @@ __global__ void __launch_bounds__(Geo<WIN>::NT, 1) sweep_kernel(const __grid_con
     }
 }
 
-/* Kernel variants: bit 0 = identity rotations, k1-only (or no) distortion, cos(fov/2) + xi >= 1e-3 (otherwise any
- * rotation, the full distortion polynomial and the denominator test); bit 1 = 8-byte bfloat16 footprints. */
+/* Kernel variants (fsw_api.cu: pick_variant): projection mode 0..2 (see SweepInst::go) + 3 if the footprints are
+ * 8-byte bfloat16. */
 template <int WIN, int NVT>
 struct SweepInst {
     using G = Geo<WIN>;
-    template <bool FAST, bool F16>
+    /* MODE 0: any rotation, full distortion polynomial, denominator test; 1: identity rotations, k1-only distortion;
+     * 2: any rotation, k1-only distortion (the last two need cos(fov/2) + xi >= 1e-3) */
+    template <int MODE, bool F16>
     static cudaError_t go(const FswSweepArgs& args, int grid, cudaStream_t stream, bool prepare_only) {
-        auto kern = sweep_kernel<WIN, NVT, FAST, !FAST, !FAST, F16>;
+        auto kern = sweep_kernel<WIN, NVT, MODE == 1, MODE == 0, MODE == 0, F16>;
         if (prepare_only) return cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::smem());
         kern<<<grid, G::NT, G::smem(), stream>>>(args);
         return cudaGetLastError();
     }
+    static constexpr int N_VARIANTS = 6;
     static cudaError_t dispatch(const FswSweepArgs& args, int variant, int grid, cudaStream_t stream, bool prep) {
-        switch (variant & 3) {
-            case 0: return go<false, false>(args, grid, stream, prep);
-            case 1: return go<true, false>(args, grid, stream, prep);
-            case 2: return go<false, true>(args, grid, stream, prep);
-            default: return go<true, true>(args, grid, stream, prep);
+        switch (variant) {
+            case 0: return go<0, false>(args, grid, stream, prep);
+            case 1: return go<1, false>(args, grid, stream, prep);
+            case 2: return go<2, false>(args, grid, stream, prep);
+            case 3: return go<0, true>(args, grid, stream, prep);
+            case 4: return go<1, true>(args, grid, stream, prep);
+            default: return go<2, true>(args, grid, stream, prep);
         }
     }
     static cudaError_t launch(const FswSweepArgs& args, int variant, int grid, cudaStream_t stream) {
@@ -829,7 +834,7 @@ struct SweepInst {
     }
     static cudaError_t prepare() {
         static const FswSweepArgs dummy = {};
-        for (int v = 0; v < 4; ++v) {
+        for (int v = 0; v < N_VARIANTS; ++v) {
             cudaError_t e = dispatch(dummy, v, 0, nullptr, true);
             if (e != cudaSuccess) return e;
         }
