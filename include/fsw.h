@@ -218,8 +218,8 @@ int32_t fsw_compute_depth(fsw_context* ctx, const fsw_planeset* planes, const fs
  * images: host array of n_sets * n_cams descriptors, set-major (images[s * n_cams + c]), device pointers.
  * masks: host array of n_sets device pointers (each nullable), or NULL for no masks; one mask_pitch for all.
  * outs: host array of n_sets output descriptors (device pointers; the sets must not alias each other).
- * 1 <= n_sets <= FSW_MAX_BATCH.  The context's footprint scratch grows to n_sets frame sets (16 bytes per view
- * pixel).  params->debug_cost_volume must be NULL unless n_sets == 1.  Asynchronous like fsw_compute_depth.
+ * 1 <= n_sets <= FSW_MAX_BATCH.  The context's footprint scratch grows to n_sets frame sets (8 bytes per view
+ * pixel for 8-bit views, 16 for float views).  params->debug_cost_volume must be NULL unless n_sets == 1.  Asynchronous like fsw_compute_depth.
  * fsw_get_last_counters then reports totals over the batch. */
 int32_t fsw_compute_depth_batch(fsw_context* ctx, const fsw_planeset* planes, const fsw_sweep_params* params,
                                 int32_t n_sets, const fsw_image* images, const uint8_t* const* masks, size_t mask_pitch,

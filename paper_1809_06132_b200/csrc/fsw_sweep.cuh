@@ -8,7 +8,7 @@
  *   and then, for every sweep plane k and every matching view,
  *   S2-S4 maps every halo pixel through the plane into the view (ray-homography form X' ~ R r + (n.r / d_k) T),
  *       projects it with the view's fisheye model and samples the view bilinearly from its footprint image (one
- *       128-bit load),
+ *       64-bit load for 8-bit views, one 128-bit load for float views),
  *   S5  forms the windowed sums of b, b^2, ab with separable sliding box sums and scores cost = (1 - ZNCC)/2
  *       (PAPER.md:76),
  *   S6  averages the cost over the views whose window is fully valid,
