@@ -609,6 +609,13 @@ __global__ void __launch_bounds__(Geo<WIN>::NT, 1) sweep_kernel(const __grid_con
                 float qmax = 0.f;
 #pragma unroll
                 for (int i = 0; i < G::NW; ++i) qmax = fmaxf(qmax, red_f[i]);
+                /* does any active output of this warp face the family at all?  If not (outside the image circle, above
+                 * the horizon for ground-parallel planes) the warp skips the vertical pass and the ZNCC of every plane */
+                bool v_act = false;
+#pragma unroll
+                for (int i = 0; i < RPT; ++i)
+                    v_act = v_act || (((active_mask >> i) & 1u) && rays[(grp * RPT + i + HW) * G::SB + col + HW].w > 0.f);
+                v_act = __any_sync(0xffffffffu, v_act);
 
 #pragma unroll 1
                 for (int j = 0; j < F.count; ++j) {
@@ -669,6 +676,10 @@ __global__ void __launch_bounds__(Geo<WIN>::NT, 1) sweep_kernel(const __grid_con
                                 ph = ph == 2 ? 0 : ph + 1;
                                 if (f_any == 0) continue; /* the view sees nothing of the tile through this plane */
                                 /* ---- vertical sums, ZNCC ------------------------------------------------------ */
+                                if (!v_act) { /* nothing to score in this warp: only keep the barrier count */
+                                    __syncthreads();
+                                    continue;
+                                }
                                 float sb[RPT], sbb[RPT], sab[RPT], sv[RPT];
                                 vpass<G, WIN>(v_src, sb);
                                 vpass<G, WIN>(v_src + G::HPLANE, sbb);
