@@ -217,7 +217,7 @@ __device__ __forceinline__ FootRaw<F16> foot_fetch(const void* __restrict__ foot
     return r;
 }
 template <bool F16>
-__device__ __forceinline__ float foot_lerp(const FootRaw<F16>& r, float au, float av, bool ok, float centre) {
+__device__ __forceinline__ float foot_lerp(const FootRaw<F16>& r, float au, float av, float centre) {
     float4 f;
     if constexpr (F16) {
         f.x = __uint_as_float(r.v.x << 16); f.y = __uint_as_float(r.v.x & 0xffff0000u);
@@ -227,8 +227,7 @@ __device__ __forceinline__ float foot_lerp(const FootRaw<F16>& r, float au, floa
     }
     float top = fmaf(au, f.y, f.x);
     float bot = fmaf(au, f.w, f.z);
-    float b = fmaf(av, bot - top, top) - centre;
-    return ok ? b : CUDART_NAN_F;
+    return fmaf(av, bot - top, top) - centre; /* NaN if au is (an invalid sample) */
 }
 
 /* NV4 * 4 consecutive floats of a sample-plane row as 128-bit loads */
@@ -384,12 +383,12 @@ __device__ __forceinline__ bool sample_rows(const float4* __restrict__ rays, flo
      * footprints of a batch stay in registers) */
     constexpr int SBATCH = (!FULLDIST && F16) ? 4 : 2;
     bool all_ok = true;
-    /* batches of SBATCH samples: all addresses, then all fetches, then the lerps */
+    /* batches of SBATCH samples: all addresses, then all fetches, then the lerps.  An invalid sample carries a NaN
+     * weight au (and fetches footprint 0 instead of branching), so its lerp yields the NaN that marks it in b_s. */
 #pragma unroll
     for (int i0 = 0; i0 < NS; i0 += SBATCH) {
         float au[SBATCH], av[SBATCH];
         unsigned idx[SBATCH];
-        unsigned okm = 0u;
         FootRaw<F16> raw[SBATCH];
 #pragma unroll
         for (int jj = 0; jj < SBATCH; ++jj) {
@@ -401,9 +400,9 @@ __device__ __forceinline__ bool sample_rows(const float4* __restrict__ rays, flo
                 s = (s >= s_min) ? s : CUDART_NAN_F;
                 SampleAddr a = sample_addr<IDENT, FULLDIST, CHECKDEN>(ry.x, ry.y, ry.z, s, view);
                 const bool on = a.ok && (i < G::NSFULL || tail_on); /* a pixel in this slot */
-                au[jj] = a.au; av[jj] = a.av;
+                au[jj] = on ? a.au : CUDART_NAN_F; av[jj] = a.av;
                 idx[jj] = on ? a.idx : 0u;
-                okm |= on ? (1u << jj) : 0u;
+                if (i < G::NSFULL || tail_on) all_ok = all_ok && on;
             }
         }
 #pragma unroll
@@ -413,12 +412,8 @@ __device__ __forceinline__ bool sample_rows(const float4* __restrict__ rays, flo
         for (int jj = 0; jj < SBATCH; ++jj) {
             const int i = i0 + jj;
             if (i < NS) {
-                const bool ok = (okm >> jj) & 1u;
-                const float b = foot_lerp<F16>(raw[jj], au[jj], av[jj], ok, centre);
-                if (i < G::NSFULL || tail_on) {
-                    b_s[sbase + 32 * i] = b;
-                    all_ok = all_ok && ok;
-                }
+                const float b = foot_lerp<F16>(raw[jj], au[jj], av[jj], centre);
+                if (i < G::NSFULL || tail_on) b_s[sbase + 32 * i] = b;
             }
         }
     }

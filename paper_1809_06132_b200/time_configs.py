@@ -5,7 +5,10 @@
 Prints one markdown table row per config: milliseconds per depth map (CUDA events on the launching stream, device
 resident inputs, 3 warm-up calls), finite cost evaluations per map (the kernel's counter) and evaluations per second.
 C1..C4 and 6 are single calls (one frame set per launch: the latency figure); C5 and the last row of 6 run 8 frame sets
-per launch like bench.py.  Inputs come from the seeded generator `synth` (no files are read)."""
+per launch like bench.py.  Config 6 is also timed on the two three-camera subsets of PAPER.md:280 (fig:camconfiguration:
+"3 Cameras (C1)" = leftmost, central, rightmost; "3 Cameras (C2)" = the three central cameras; the paper reports that
+they "save about 17% of run time"): a subset is simply a rig built from those cameras.
+Inputs come from the seeded generator `synth` (no files are read)."""
 from __future__ import annotations
 
 import argparse
@@ -43,13 +46,22 @@ def main():
 
     print("| config | call | ms per depth map | finite cost evaluations per map | evaluations / s |")
     print("|---|---|---|---|---|")
-    for idx in (1, 2, 3, 4, 5, 6):
+    # (config index, camera subset or None, label suffix); the rig of config 6 is (reference = central, outer left,
+    # outer right, inner left, inner right)
+    runs = [(i, None, "") for i in (1, 2, 3, 4, 5, 6)] + [(6, (0, 1, 2), " 3 cameras (C1)"), (6, (0, 3, 4), " 3 cameras (C2)")]
+    for idx, subset, suffix in runs:
         cfg = synth.make_config(idx)
+        if subset is not None:
+            cfg = dict(cfg, cams=[cfg["cams"][i] for i in subset], name=cfg["name"] + suffix)
         rig = fsw.Rig(cfg["cams"], cfg["ref_index"])
         ctx = fsw.Context(rig, 0)
         W, H = cfg["cams"][0]["width"], cfg["cams"][0]["height"]
         n_frames = 8 if idx >= 5 else 1
         frames = [[torch.from_numpy(im).cuda() for im in synth.render_frame(cfg, f)] for f in range(n_frames)]
+        if subset is not None:
+            rows_filter = lambda rows: rows[-1:]  # the batched row only
+        else:
+            rows_filter = lambda rows: rows
         if idx == 4:
             pl, pc = fsw.PlaneSet(cfg["families_low"]), fsw.PlaneSet(cfg["families_crop"])
             mask = torch.from_numpy(synth.make_mask(W, H, cfg["mask_seed"])).cuda()
@@ -64,7 +76,7 @@ def main():
             if n_frames > 1:
                 rows.append(("fsw_compute_depth_batch, 8 frame sets",
                              lambda: ctx.compute_depth_batch(planes, cfg["params"], frames, masks), n_frames))
-        for label, fn, n in rows:
+        for label, fn, n in rows_filter(rows):
             ms = timed(fn, args.reps) / n
             n_eval = ctx.last_counters()["n_eval"] / n
             print("| %s %dx%d | %s | %.4f | %.4g | %.3g |" % (cfg["name"], W, H, label, ms, n_eval, n_eval / (ms * 1e-3)))
