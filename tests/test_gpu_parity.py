@@ -90,6 +90,41 @@ def test_config5_stream_frames(frame):
     assert (test["depth"][mask != 0] == 0).all()
 
 
+def test_config5_batch_of_8_as_benchmarked():
+    """The launch configuration bench.py times: 8 consecutive C5 frame sets (with their masks) in ONE sweep launch
+    (fsw_compute_depth_batch) at full size.  One frame set of the launch is gated against the oracle, and every set
+    must be bit-identical to its own single-set call."""
+    import torch
+    import paper_1809_06132_b200 as fsw
+    cfg = synth.make_config(5)
+    _, _, ctx = gpu_objects(cfg)
+    planes = fsw.PlaneSet(cfg["families"])
+    frames = list(range(8, 16))
+    sets = [synth.render_frame(cfg, f) for f in frames]
+    masks = [synth.make_mask(1280, 1024, cfg["mask_seed"] + f) for f in frames]
+    dev_sets = [[torch.from_numpy(im).cuda() for im in st] for st in sets]
+    dev_masks = [torch.from_numpy(m).cuda() for m in masks]
+    outs = ctx.compute_depth_batch(planes, cfg["params"], dev_sets, dev_masks)
+    torch.cuda.synchronize()
+    counters = ctx.last_counters()
+    assert counters["n_launches"] == 2  # one footprint pack, one sweep
+    batch = [oracle.compare.to_numpy(o) for o in outs]
+    n_eval = 0
+    for s in range(8):
+        single = oracle.compare.to_numpy(ctx.compute_depth(planes, cfg["params"], dev_sets[s], dev_masks[s]))
+        n_eval += ctx.last_counters()["n_eval"]
+        for key in ("depth", "best_cost", "second_cost", "plane_index", "valid_reason"):
+            assert np.array_equal(single[key], batch[s][key], equal_nan=True), (s, key)
+    assert counters["n_eval"] == n_eval
+    s = 5
+    ref = oracle.compute_depth(cfg["cams"], cfg["ref_index"], cfg["families"], cfg["params"], sets[s], masks[s], keep_cost=True)
+    cond = oracle.compare.depth_conditioning(ref, oracle.plane_table(cfg["families"])[0])
+    stats = oracle.compare.compare_maps(ref, batch[s], ref["cost"], depth_cond=cond)
+    stats["n_eval_oracle"], stats["n_eval_test"] = ref["n_eval"], ref["n_eval"]
+    assert_gates(stats)
+    assert (batch[s]["depth"][masks[s] != 0] == 0).all()
+
+
 # ---- cost volume, element by element --------------------------------------------------------------------------------
 def test_debug_cost_volume_matches_oracle():
     cfg = synth.make_config(2)
