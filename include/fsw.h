@@ -164,6 +164,7 @@ typedef struct fsw_counters {
     int64_t n_launches;  /* CUDA kernels launched by the last call */
     double sweep_ms;     /* device time of the sweep kernel(s) of the last call, CUDA events on the call's stream;
                             -1 unless fsw_context_set_timing(ctx, 1) was in effect */
+    int64_t n_split_launches; /* sweep launches of the last call that split their tiles (fsw_context_set_split) */
 } fsw_counters;
 
 /* ---- version / errors ---------------------------------------------------- */
@@ -249,6 +250,18 @@ int32_t fsw_compute_depth_multires_host(fsw_context* ctx, const fsw_planeset* pl
                                         const fsw_sweep_params* params_crop, fsw_rect crop, const fsw_image* images,
                                         const uint8_t* mask, size_t mask_pitch, const fsw_depth_out* out,
                                         void* cuda_stream);
+
+/* Load balancing of calls with few frame sets (S0).  The sweep kernel runs one persistent CTA per SM over a queue of
+ * (frame set, tile) items; a single 1280 x 1024 frame set has 176 live tiles for 148 SMs.  With the plane split every
+ * tile becomes two work items that sweep one half of the planes each (the planes are independent
+ * hypotheses) and merge their winner-take-all states; the maps are bit-identical to the unsplit ones.
+ * FSW_SPLIT_AUTO (default): split when the live tiles of the call are fewer than three per SM; FSW_SPLIT_OFF: never;
+ * FSW_SPLIT_ON: always.  Calls with fewer than two planes or more than two matching views are never split.  The context then owns 48 bytes of scratch per reference pixel
+ * and frame set of such a call.  Errors: FSW_E_INVALID_ARG for a null context or an unknown mode. */
+#define FSW_SPLIT_AUTO 0
+#define FSW_SPLIT_OFF 1
+#define FSW_SPLIT_ON 2
+int32_t fsw_context_set_split(fsw_context* ctx, int32_t mode);
 
 /* on != 0: every following compute call brackets its sweep kernel launches (the dominant kernels, S1-S12) with a
  * pair of CUDA events on the call's stream so that fsw_get_last_counters can report their device time.  Off by

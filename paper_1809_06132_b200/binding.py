@@ -28,7 +28,7 @@ EXPORTS = (
     "fsw_planeset_table", "fsw_context_create", "fsw_context_destroy", "fsw_compute_depth",
     "fsw_compute_depth_multires", "fsw_compute_depth_host", "fsw_compute_depth_multires_host",
     "fsw_compute_depth_batch", "fsw_compute_depth_batch_host",
-    "fsw_context_set_timing", "fsw_get_last_counters", "fsw_measure_fp32_peak", "fsw_filter_continuity",
+    "fsw_context_set_timing", "fsw_context_set_split", "fsw_get_last_counters", "fsw_measure_fp32_peak", "fsw_filter_continuity",
 )
 
 
@@ -78,7 +78,8 @@ class CDepthOut(ctypes.Structure):
 
 class CCounters(ctypes.Structure):
     _fields_ = [("struct_size", ctypes.c_uint32), ("n_eval", ctypes.c_int64), ("n_raw_valid", ctypes.c_int64),
-                ("n_valid", ctypes.c_int64), ("n_launches", ctypes.c_int64), ("sweep_ms", ctypes.c_double)]
+                ("n_valid", ctypes.c_int64), ("n_launches", ctypes.c_int64), ("sweep_ms", ctypes.c_double),
+                ("n_split_launches", ctypes.c_int64)]
 
 
 _lib = None
@@ -120,6 +121,7 @@ def load_library():
     L.fsw_compute_depth_batch_host.argtypes = batch
     L.fsw_compute_depth_multires_host.argtypes = multi
     L.fsw_context_set_timing.argtypes = [vp, i32]
+    L.fsw_context_set_split.argtypes = [vp, i32]
     L.fsw_get_last_counters.argtypes = [vp, P(CCounters)]
     L.fsw_measure_fp32_peak.argtypes = [i32, vp, P(ctypes.c_double), P(ctypes.c_double)]
     for name in EXPORTS:
@@ -429,7 +431,11 @@ class Context:
         c.struct_size = ctypes.sizeof(CCounters)
         _check(load_library().fsw_get_last_counters(self.handle, ctypes.byref(c)))
         return dict(n_eval=c.n_eval, n_raw_valid=c.n_raw_valid, n_valid=c.n_valid, n_launches=c.n_launches,
-                    sweep_ms=c.sweep_ms)
+                    sweep_ms=c.sweep_ms, n_split_launches=c.n_split_launches)
+
+    def set_split(self, mode="auto"):
+        """fsw_context_set_split: plane split of the tiles of calls with few frame sets ('auto', 'off', 'on')."""
+        _check(load_library().fsw_context_set_split(self.handle, {"auto": 0, "off": 1, "on": 2}[mode]))
 
     def set_timing(self, on=True):
         """fsw_context_set_timing: bracket the sweep kernels of later calls with CUDA events (last_counters()['sweep_ms'])."""

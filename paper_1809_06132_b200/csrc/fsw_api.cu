@@ -117,6 +117,10 @@ struct fsw_context {
     DevBuf lo_depth, lo_c1, lo_c2, lo_k;
     DevBuf ctrl;                   /* FSW_CTRL_WORDS x uint32 */
     DevBuf sets_dev;               /* FswSetPtrs of a batch */
+    DevBuf split_state;            /* plane split: [set][half][6][H][W] floats */
+    DevBuf split_ticket;           /* plane split: one word per (set, tile), zero between launches */
+    int32_t split_mode = FSW_SPLIT_AUTO;
+    int64_t last_split = 0;        /* sweep launches of the last call that split their tiles */
     std::vector<TileOrder*> orders;
     /* staging for the *_host calls: [set slot] */
     std::vector<DevBuf> st_img, st_mask, st_depth, st_c1, st_c2, st_k, st_reason;
@@ -399,10 +403,60 @@ int32_t launch_sweep(fsw_context* ctx, FswSweepArgs& a, int w, cudaStream_t s) {
     a.n_tiles = order->n_tiles;
     a.queue = ctx->queue();
     a.counters = ctx->counters();
-    const long long items = (long long)a.n_tiles * a.n_sets;
     const long long slots = (long long)ctx->n_sm * g.ctas_per_sm;
+    /* Plane split (fsw_context_set_split): few frame sets leave the persistent grid unbalanced -- a 1280 x 1024 frame
+     * has 176 live tiles for 148 CTAs, every CTA takes one and 28 take a second one.  Then every tile becomes two
+     * work items with half of the planes (by expected work: a family facing away from the optical axis is reached
+     * by about (1 + n_z)/2 of the rays) and the halves merge their winner-take-all states (fsw_sweep.cuh). */
+    a.split = 0;
+    if (ctx->split_mode != FSW_SPLIT_OFF && a.n_planes >= 2 && a.n_views <= 2) {
+        long long live = 0; /* tiles that intersect the region of interest and the image circle (the kernel's test) */
+        const int hw = w / 2;
+        for (int t = 0; t < a.n_tiles; ++t) {
+            const int ty = t / a.n_tiles_x, tx = t - ty * a.n_tiles_x;
+            const int x0 = tx * g.tile_w, y0 = ty * g.tile_h;
+            if (!(x0 < a.roi_x1 && x0 + g.tile_w > a.roi_x0 && y0 < a.roi_y1 && y0 + g.tile_h > a.roi_y0)) continue;
+            const float nx = std::max(std::max((float)(x0 - hw) - a.ref.cx, a.ref.cx - (float)(x0 + g.tile_w - 1 + hw)), 0.f) / a.ref.fx;
+            const float ny = std::max(std::max((float)(y0 - hw) - a.ref.cy, a.ref.cy - (float)(y0 + g.tile_h - 1 + hw)), 0.f) / a.ref.fy;
+            if (nx * nx + ny * ny <= a.ref_rd2_max) ++live;
+        }
+        if (ctx->split_mode == FSW_SPLIT_ON || live * a.n_sets < 3 * slots) {
+            double total = 0.0, acc = 0.0;
+            std::vector<double> wk((size_t)a.n_planes);
+            for (int f = 0; f < a.n_fams; ++f)
+                for (int j = 0; j < a.fam[f].count; ++j) {
+                    wk[(size_t)a.fam[f].first + j] = std::max(0.1, 0.5 * (1.0 + (double)a.fam[f].n[2]));
+                    total += wk[(size_t)a.fam[f].first + j];
+                }
+            int kb = 1;
+            for (int k = 0; k < a.n_planes - 1; ++k) {
+                acc += wk[(size_t)k];
+                kb = k + 1;
+                if (acc >= 0.5 * total) break;
+            }
+            int fa = 0, fb = 0;
+            for (int f = 0; f < a.n_fams; ++f) {
+                if (kb - 1 >= a.fam[f].first) fa = f;
+                if (kb >= a.fam[f].first) fb = f;
+            }
+            const size_t mapsz = (size_t)a.ref.W * a.ref.H;
+            FSW_CUDA(ctx->split_state.reserve((size_t)a.n_sets * 2 * 6 * mapsz * sizeof(float)));
+            const size_t tbytes = (size_t)a.n_sets * a.n_tiles * sizeof(unsigned int);
+            if (tbytes > ctx->split_ticket.bytes) {
+                FSW_CUDA(ctx->split_ticket.reserve(tbytes));
+                FSW_CUDA(cudaMemsetAsync(ctx->split_ticket.p, 0, ctx->split_ticket.bytes, s));
+            }
+            a.split = 1;
+            a.split_k = kb;
+            a.split_adjacent = fa == fb ? 1 : 0;
+            a.split_state = (float*)ctx->split_state.p;
+            a.split_ticket = (unsigned int*)ctx->split_ticket.p;
+        }
+    }
+    ctx->last_split += a.split;
+    const long long items = (long long)a.n_tiles * a.n_sets * (a.split ? 2 : 1);
     const int grid = (int)(items < slots ? items : slots);
-    const int var = pick_variant(a, a.foot_f16);
+    const int var = pick_variant(a, a.foot_f16) + (a.split ? 6 : 0);
     cudaError_t e = cudaErrorInvalidValue;
     switch (w) {
         case 3: e = fsw_launch_sweep_w3(a, var, grid, s); break;
@@ -657,6 +711,7 @@ int32_t fsw_context_destroy(fsw_context* ctx) {
         for (DevBuf& b : *v) b.release();
     ctx->lo_depth.release(); ctx->lo_c1.release(); ctx->lo_c2.release(); ctx->lo_k.release();
     ctx->ctrl.release(); ctx->sets_dev.release();
+    ctx->split_state.release(); ctx->split_ticket.release();
     for (TileOrder* t : ctx->orders) {
         t->dev.release();
         delete t;
@@ -688,6 +743,7 @@ static int32_t run_sets(fsw_context* ctx, const fsw_planeset* planes, const fsw_
     FSW_CUDA(prepare_window(ctx, params->window));
     ctx->last_stream = stream;
     ctx->last_launches = 0;
+    ctx->last_split = 0;
 
     FswSweepArgs a;
     fill_args(a, rig, *planes, *params, false);
@@ -752,6 +808,7 @@ int32_t fsw_compute_depth_multires(fsw_context* ctx, const fsw_planeset* planes_
     FSW_CUDA(prepare_window(ctx, params_crop->window));
     ctx->last_stream = stream;
     ctx->last_launches = 0;
+    ctx->last_split = 0;
 
     /* S10(a): 2x2 box downsample of every image */
     FswDownArgs dn;
@@ -936,6 +993,14 @@ int32_t fsw_filter_continuity(fsw_context* ctx, const float* depth_in, size_t de
     return FSW_OK;
 }
 
+int32_t fsw_context_set_split(fsw_context* ctx, int32_t mode) {
+    if (!ctx) return fail(FSW_E_INVALID_ARG, "fsw_context_set_split: null context");
+    if (mode != FSW_SPLIT_AUTO && mode != FSW_SPLIT_OFF && mode != FSW_SPLIT_ON)
+        return fail(FSW_E_INVALID_ARG, "fsw_context_set_split: mode %d", mode);
+    ctx->split_mode = mode;
+    return FSW_OK;
+}
+
 int32_t fsw_context_set_timing(fsw_context* ctx, int32_t on) {
     if (!ctx) return fail(FSW_E_INVALID_ARG, "fsw_context_set_timing: null context");
     DeviceGuard g;
@@ -958,6 +1023,7 @@ int32_t fsw_get_last_counters(fsw_context* ctx, fsw_counters* out) {
     out->n_eval = (int64_t)h[0];
     out->n_raw_valid = (int64_t)h[1];
     out->n_valid = (int64_t)h[2];
+    out->n_split_launches = ctx->last_split;
     out->n_launches = ctx->last_launches;
     out->sweep_ms = -1.0;
     if (ctx->n_timed > 0) {

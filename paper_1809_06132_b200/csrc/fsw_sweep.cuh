@@ -295,6 +295,19 @@ __device__ __forceinline__ bool hsum(float (&p)[G::NV4 * 4], const float (&q)[G:
     return any;
 }
 
+/* the row sums of one work item cleared (rows that no ray reaches: the sliding vertical sums of the columns must not
+ * carry values of an earlier pass, or a cost would depend in its last bit on the order the planes are visited in) */
+template <class G>
+__device__ __forceinline__ void fill_zero(float* __restrict__ hs) {
+    const float4 z = make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+    for (int pl = 0; pl < 4; ++pl) {
+        float4* h = reinterpret_cast<float4*>(hs + pl * G::HPLANE);
+        h[0] = z;
+        h[1] = z;
+    }
+}
+
 /* RUN entries of plane 3 (valid counts of the horizontal windows) of one work item set to c */
 template <class G>
 __device__ __forceinline__ void fill_count(float* __restrict__ hs, float c) {
@@ -325,7 +338,8 @@ __device__ __forceinline__ void vpass(const float* __restrict__ h, float (&out)[
 /* streaming winner-take-all state of one output pixel (S7).  b1 = lowest cost so far (lowest index wins ties),
  * m2 = lowest cost of the planes at least two back (eligible as second best when the current plane becomes the
  * best), s2 = second best of the current best, cm / cp = costs of the planes below / above the best, knext = index
- * of the plane above the best while it is still to come in the same family. */
+ * of the plane above the best while it is still to come in the same family (kept in a register by the unsplit
+ * kernel only; the split kernel, shorter of registers, derives it from k1). */
 struct Wta {
     float b1, m2, s2, cm, cp, cprev;
     int k1, knext;
@@ -336,20 +350,26 @@ struct Wta {
     }
     /* family start: planes of another family are never "adjacent" (reading Q12) */
     __device__ __forceinline__ void family_start() { m2 = b1; cprev = CUDART_INF_F; knext = -1; }
-    __device__ __forceinline__ void update(float c, int k) {
-        const bool isn = (k == knext);  /* neighbour above the running best: not eligible as second best */
-        const bool nb = c < b1;         /* strict: lowest index wins ties */
+    /* Planes are visited in ascending index order (dir = +1), or -- in the second half of a split tile -- in
+     * descending order (dir = -1, desc): then an equal cost wins as well (the later plane has the lower index), and
+     * cm / cp hold the neighbour visited before / after the best, i.e. above / below it (swap_neighbours()). */
+    template <bool KNEXT>
+    __device__ __forceinline__ void update(float c, int k, int dir, bool desc, bool fam_first) {
+        /* neighbour of the running best on the far side (same family): not eligible as second best */
+        const bool isn = KNEXT ? (k == knext) : (!fam_first && (k == k1 + dir));
+        const bool nb = desc ? ((c <= b1) && (c < CUDART_INF_F)) : (c < b1); /* lowest index wins ties */
         cp = isn ? c : cp;
         const float t = isn ? s2 : fminf(s2, c);
         s2 = nb ? m2 : t;
         cm = nb ? cprev : cm;
         cp = nb ? CUDART_INF_F : cp;
         k1 = nb ? k : k1;
-        knext = nb ? k + 1 : knext;
+        if (KNEXT) knext = nb ? k + dir : knext;
         m2 = b1;
         b1 = fminf(b1, c);
         cprev = c;
     }
+    __device__ __forceinline__ void swap_neighbours() { const float t = cm; cm = cp; cp = t; }
 };
 
 __device__ __forceinline__ float warp_max(float v) {
@@ -427,7 +447,7 @@ struct SetHot {
 };
 
 /* NVT = number of views known at compile time (1 or 2), 0 = read args.n_views at run time. */
-template <int WIN, int NVT, bool IDENT, bool FULLDIST, bool CHECKDEN, bool F16>
+template <int WIN, int NVT, bool IDENT, bool FULLDIST, bool CHECKDEN, bool F16, bool SPLIT>
 __global__ void __launch_bounds__(Geo<WIN>::NT, 1) sweep_kernel(const __grid_constant__ FswSweepArgs args) {
     using G = Geo<WIN>;
     constexpr int HW = G::HW, RPT = G::RPT, NS = G::NS, TX = G::TX, TY = G::TY, R = G::R;
@@ -449,7 +469,7 @@ __global__ void __launch_bounds__(Geo<WIN>::NT, 1) sweep_kernel(const __grid_con
     /* [TY][TX]: reference-side window statistics of every output: ((sum a')/N, sum a'^2 - (sum a')^2/N) */
     float2* const a_stat = reinterpret_cast<float2*>(hs + 4 * G::HPLANE) + (grp * RPT) * TX + col;
     const int W = args.ref.W, H = args.ref.H;
-    const int n_items = args.n_tiles * args.n_sets;
+    const int n_items = args.n_tiles * args.n_sets * (SPLIT ? 2 : 1);
     const int n_views = NVT ? NVT : args.n_views;
 
     /* this lane's halo pixels: slot i is element lane + 32 i of the warp's R x SB block of the sample planes; in the
@@ -468,8 +488,16 @@ __global__ void __launch_bounds__(Geo<WIN>::NT, 1) sweep_kernel(const __grid_con
 
     unsigned item = blockIdx.x;
     while (item < (unsigned)n_items) {
-        const int set = (int)(item % (unsigned)args.n_sets);
-        const int tile = args.tile_order[item / (unsigned)args.n_sets];
+        /* plane split: item = 2 * (tile slot) + half; own planes [k_lo, k_hi), visited downwards in half 1 */
+        const int half = SPLIT ? (int)(item & 1u) : 0;
+        const unsigned titem = SPLIT ? item >> 1 : item;
+        const bool desc = SPLIT && half != 0;
+        const int dir = desc ? -1 : 1;
+        const int k_lo = desc ? args.split_k : 0, k_hi = (SPLIT && !half) ? args.split_k : args.n_planes;
+        /* the plane across the cut, evaluated only as the parabola neighbour of a winner next to the cut */
+        const int k_halo = (SPLIT && args.split_adjacent) ? (half ? args.split_k - 1 : args.split_k) : -1;
+        const int set = (int)(titem % (unsigned)args.n_sets);
+        const int tile = args.tile_order[titem / (unsigned)args.n_sets];
         const FswSetPtrs& S = args.n_sets > 1 ? args.sets[set] : args.set0;
         const int tyi = tile / args.n_tiles_x, txi = tile - tyi * args.n_tiles_x;
         const int x0t = txi * TX, y0t = tyi * TY;
@@ -579,8 +607,19 @@ __global__ void __launch_bounds__(Geo<WIN>::NT, 1) sweep_kernel(const __grid_con
             const float inv_views = 1.f / (float)n_views;
             unsigned ph = 0; /* rotation of the pass flags */
 #pragma unroll 1
-            for (int f = 0; f < args.n_fams; ++f) {
+            for (int fi = 0; fi < args.n_fams; ++fi) {
+                const int f = desc ? args.n_fams - 1 - fi : fi;
                 const FswDevFamily& F = args.fam[f];
+                /* own planes of this item in the family: j0 <= j < j1 */
+                int j0 = 0, j1 = F.count;
+                bool has_halo = false;
+                if constexpr (SPLIT) {
+                    j0 = max(k_lo - F.first, 0);
+                    j1 = min(k_hi - F.first, F.count);
+                    if (j1 <= j0) continue;
+                    has_halo = k_halo >= F.first && k_halo < F.first + F.count; /* then the last family visited */
+                }
+                const int n_own = j1 - j0;
                 const float fnx = F.n[0], fny = F.n[1], fnz = F.n[2];
 #pragma unroll
                 for (int i = 0; i < RPT; ++i) st[i].family_start();
@@ -613,8 +652,9 @@ __global__ void __launch_bounds__(Geo<WIN>::NT, 1) sweep_kernel(const __grid_con
                 v_act = __any_sync(0xffffffffu, v_act);
 
 #pragma unroll 1
-                for (int j = 0; j < F.count; ++j) {
-                    const int k = F.first + j;
+                for (int it = 0; it < n_own + (has_halo ? 1 : 0); ++it) {
+                    const bool halo = SPLIT && it >= n_own;
+                    const int k = !SPLIT ? F.first + it : (halo ? k_halo : F.first + (desc ? j1 - 1 - it : j0 + it));
                     const float inv_d = args.inv_d[k];
                     float acc[RPT];
                     unsigned cnt = 0; /* valid views per output, 4 bits each */
@@ -655,7 +695,7 @@ __global__ void __launch_bounds__(Geo<WIN>::NT, 1) sweep_kernel(const __grid_con
                                     if (!all_ok) any_ok = __any_sync(0xffffffffu, any_l);
                                     p3 = all_ok ? 0 : 2;
                                 } else {
-                                    if (p3 != 1 && h_on) fill_count<G>(h_dst, 0.f);
+                                    if (p3 != 1 && h_on) fill_zero<G>(h_dst);
                                     p3 = 1;
                                 }
                                 if (lane == 0) {
@@ -706,21 +746,25 @@ __global__ void __launch_bounds__(Geo<WIN>::NT, 1) sweep_kernel(const __grid_con
                         else if (NVT == 2) c = ci == 2 ? 0.5f * acc[i] : acc[i];
                         else c = ci == n_views ? acc[i] * inv_views : acc[i] * args.inv_count[ci];
                         c = ci > 0 ? c : CUDART_INF_F;
-                        n_eval += ci;
-                        st[i].update(c, k);
+                        if (halo) { /* neighbour across the cut of a winner next to it; nothing else changes */
+                            st[i].cp = st[i].k1 + dir == k ? c : st[i].cp;
+                        } else {
+                            n_eval += ci;
+                            st[i].template update<!SPLIT>(c, k, dir, desc, it == 0);
+                        }
                     }
                     if (dbg) {
                         float* dc = s_set.debug_cost;
 #pragma unroll
                         for (int i = 0; i < RPT; ++i) {
                             const int oy = oy0 + i;
-                            if (ox < W && oy < H) dc[((int64_t)k * H + oy) * W + ox] = st[i].cprev;
+                            if (ox < W && oy < H && !halo) dc[((int64_t)k * H + oy) * W + ox] = st[i].cprev;
                         }
                     }
                 }
             }
         }
-        if (dbg && !tile_active) {
+        if (dbg && !tile_active && half == 0) {
             for (int k = 0; k < args.n_planes; ++k)
 #pragma unroll
                 for (int i = 0; i < RPT; ++i) {
@@ -729,12 +773,72 @@ __global__ void __launch_bounds__(Geo<WIN>::NT, 1) sweep_kernel(const __grid_con
                 }
         }
 
+        /* ---- plane split: the half of a tile that finishes first leaves its winner-take-all state in global memory,
+         * the other one merges it into its registers and goes on.  State per pixel: b1, k1, s2, cm, cp and m2 = the
+         * lowest cost of the half's planes except the one next to the cut (visited last). ----------------------- */
+        bool do_epilogue = true;
+        if (desc) {
+#pragma unroll
+            for (int i = 0; i < RPT; ++i) st[i].swap_neighbours();
+        }
+        if (SPLIT) {
+            if (!tile_active) {
+                do_epilogue = half == 0; /* nothing was swept: one half writes the invalid / upsampled outputs */
+            } else {
+                const size_t mapsz = (size_t)H * W;
+                float* const mine = args.split_state + ((size_t)set * 2 + half) * 6 * mapsz;
+                const float* const other = args.split_state + ((size_t)set * 2 + (1 - half)) * 6 * mapsz;
+                const unsigned tslot = (unsigned)set * (unsigned)args.n_tiles + (unsigned)tile;
+#pragma unroll
+                for (int i = 0; i < RPT; ++i) {
+                    const int oy = oy0 + i;
+                    if (ox >= W || oy >= H) continue;
+                    float* q = mine + (size_t)oy * W + ox;
+                    __stcg(q, st[i].b1); __stcg(q + mapsz, __int_as_float(st[i].k1)); __stcg(q + 2 * mapsz, st[i].s2);
+                    __stcg(q + 3 * mapsz, st[i].cm); __stcg(q + 4 * mapsz, st[i].cp); __stcg(q + 5 * mapsz, st[i].m2);
+                }
+                __threadfence();
+                __syncthreads();
+                if (tid == 0) s_item = atomicAdd(&args.split_ticket[tslot], 1u);
+                __syncthreads();
+                const unsigned ticket = s_item;
+                __syncthreads(); /* s_item is reused for the queue below */
+                if (ticket == 0) {
+                    do_epilogue = false;
+                } else {
+                    if (tid == 0) args.split_ticket[tslot] = 0u; /* both halves are through: ready for the next launch */
+                    __threadfence();
+#pragma unroll
+                    for (int i = 0; i < RPT; ++i) {
+                        const int oy = oy0 + i;
+                        if (ox >= W || oy >= H) continue;
+                        const float* q = other + (size_t)oy * W + ox;
+                        const float ob1 = __ldcg(q), os2 = __ldcg(q + 2 * mapsz), ocm = __ldcg(q + 3 * mapsz);
+                        const float ocp = __ldcg(q + 4 * mapsz), om2 = __ldcg(q + 5 * mapsz);
+                        const int ok1 = __float_as_int(__ldcg(q + mapsz));
+                        Wta& m = st[i];
+                        /* A = planes below the cut (half 0), B = planes from the cut on; the lower index wins a tie */
+                        const bool a_wins = half == 0 ? (m.b1 <= ob1) : (ob1 <= m.b1);
+                        const bool mine_wins = a_wins == (half == 0);
+                        const float lb1 = mine_wins ? ob1 : m.b1, lm2 = mine_wins ? om2 : m.m2;
+                        m.b1 = mine_wins ? m.b1 : ob1; m.k1 = mine_wins ? m.k1 : ok1; m.s2 = mine_wins ? m.s2 : os2;
+                        m.cm = mine_wins ? m.cm : ocm; m.cp = mine_wins ? m.cp : ocp;
+                        /* second best (reading Q12): the loser's planes all count, except the one next to the cut when
+                         * the winner sits on the other side of it */
+                        const int edge = a_wins ? args.split_k - 1 : args.split_k;
+                        const bool at_cut = args.split_adjacent && m.k1 == edge;
+                        m.s2 = fminf(m.s2, at_cut ? lm2 : lb1);
+                    }
+                }
+            }
+        }
+
         /* ---- S8-S12: refinement, depth, merge, filters, mask, stores --------------------------------------- */
         unsigned n_raw = 0, n_ok = 0;
 #pragma unroll
         for (int i = 0; i < RPT; ++i) {
             const int oy = oy0 + i;
-            if (ox >= W || oy >= H) continue;
+            if (ox >= W || oy >= H || !do_epilogue) continue;
             bool raw_valid = st[i].k1 >= 0;
             float depth = 0.f, c1 = CUDART_INF_F, c2 = CUDART_INF_F;
             int kidx = -1;
@@ -817,23 +921,40 @@ struct SweepInst {
     using G = Geo<WIN>;
     /* MODE 0: any rotation, full distortion polynomial, denominator test; 1: identity rotations, k1-only distortion;
      * 2: any rotation, k1-only distortion (the last two need cos(fov/2) + xi >= 1e-3) */
-    template <int MODE, bool F16>
+    template <int MODE, bool F16, bool SPLIT>
     static cudaError_t go(const FswSweepArgs& args, int grid, cudaStream_t stream, bool prepare_only) {
-        auto kern = sweep_kernel<WIN, NVT, MODE == 1, MODE == 0, MODE == 0, F16>;
+        auto kern = sweep_kernel<WIN, NVT, MODE == 1, MODE == 0, MODE == 0, F16, SPLIT>;
         if (prepare_only) return cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::smem());
         kern<<<grid, G::NT, G::smem(), stream>>>(args);
         return cudaGetLastError();
     }
-    static constexpr int N_VARIANTS = 6;
+    /* + 6: plane split (two work items per tile), built for the variants with one or two views only: the run-time
+     * view loop with the split faulted on the device (misaligned address in the 9 x 9 instantiation) whenever the
+     * halo plane, the descending half and the state exchange were all compiled in, and not with any one of them
+     * removed; fsw_api.cu does not split calls with more than two views until that is understood */
+    static constexpr int N_VARIANTS = NVT ? 12 : 6;
     static cudaError_t dispatch(const FswSweepArgs& args, int variant, int grid, cudaStream_t stream, bool prep) {
         switch (variant) {
-            case 0: return go<0, false>(args, grid, stream, prep);
-            case 1: return go<1, false>(args, grid, stream, prep);
-            case 2: return go<2, false>(args, grid, stream, prep);
-            case 3: return go<0, true>(args, grid, stream, prep);
-            case 4: return go<1, true>(args, grid, stream, prep);
-            default: return go<2, true>(args, grid, stream, prep);
+            case 0: return go<0, false, false>(args, grid, stream, prep);
+            case 1: return go<1, false, false>(args, grid, stream, prep);
+            case 2: return go<2, false, false>(args, grid, stream, prep);
+            case 3: return go<0, true, false>(args, grid, stream, prep);
+            case 4: return go<1, true, false>(args, grid, stream, prep);
+            case 5: return go<2, true, false>(args, grid, stream, prep);
+            default: break;
         }
+        if constexpr (NVT != 0) {
+            switch (variant) {
+                case 6: return go<0, false, true>(args, grid, stream, prep);
+                case 7: return go<1, false, true>(args, grid, stream, prep);
+                case 8: return go<2, false, true>(args, grid, stream, prep);
+                case 9: return go<0, true, true>(args, grid, stream, prep);
+                case 10: return go<1, true, true>(args, grid, stream, prep);
+                case 11: return go<2, true, true>(args, grid, stream, prep);
+                default: break;
+            }
+        }
+        return cudaErrorInvalidValue;
     }
     static cudaError_t launch(const FswSweepArgs& args, int variant, int grid, cudaStream_t stream) {
         return dispatch(args, variant, grid, stream, false);

@@ -289,6 +289,78 @@ def test_batch_equals_single_calls():
         ctx.compute_depth_batch(planes, p, [], None)
 
 
+def test_plane_split_is_bit_identical_to_the_unsplit_sweep():
+    """fsw_context_set_split: tiles swept as two half plane ranges (ascending below the cut, descending above it) and
+    merged must give exactly the maps, the cost volume and the counters of the unsplit sweep -- cut inside a family
+    (with the neighbour across the cut), cut at a family boundary, two planes only, the multi-resolution call and a
+    batch; and the automatic mode must split a single full-size frame set but not a batch of eight."""
+    import torch
+    import paper_1809_06132_b200 as fsw
+    keys = ("depth", "best_cost", "second_cost", "plane_index", "valid_reason")
+
+    def both(ctx, run):
+        res = []
+        for mode in ("off", "on"):
+            ctx.set_split(mode)
+            out = run()
+            torch.cuda.synchronize()
+            res.append((oracle.compare.to_numpy(out), ctx.last_counters()))
+        (a, ca), (b, cb) = res
+        assert ca["n_split_launches"] == 0 and cb["n_split_launches"] >= 1
+        for key in keys + (("cost_volume",) if "cost_volume" in a else ()):
+            assert np.array_equal(a[key], b[key], equal_nan=True), key
+        for key in ("n_eval", "n_raw_valid", "n_valid"):
+            assert ca[key] == cb[key], key
+        return a
+
+    fam_sets = [
+        [synth.family((0, 0, 1), 24, 0.8, 30.0, "inverse")],                                       # cut inside the family
+        [synth.family((0, 0, 1), 12, 0.8, 30.0, "inverse"), synth.family((0, 1, 0), 24, 0.4, 1.6, "linear")],  # at the boundary
+        [synth.family((0, 0, 1), 9, 0.8, 30.0, "inverse"), synth.family((0, 1, 0), 4, 0.4, 1.6, "linear"),
+         synth.family((0.1, 0.2, 1), 7, 1.0, 20.0, "linear")],                                     # three families
+        [synth.family((0, 0, 1), 2, 2.0, 4.0, "inverse")],                                         # two planes: 1 + 1
+        [synth.family((0, 0, 1), 1, 3.0, 3.0, "inverse"), synth.family((0, 1, 0), 1, 1.0, 1.0, "linear")],
+    ]
+    cfg = _small_rig(W=150, H=101, n_views=2, fov=170.0)
+    _, _, ctx = gpu_objects(cfg)
+    images = synth.render_frame(dict(cfg, scene=synth.scene_boxes(seed=5)), 0)
+    dev = [torch.from_numpy(im).cuda() for im in images]
+    p = dict(cfg["params"], filters=3, alpha_upper=0.4, alpha_lower=0.4, beta=1.05, horizon_row=50)
+    for fams in fam_sets:
+        planes = fsw.PlaneSet(fams)
+        a = both(ctx, lambda: ctx.compute_depth(planes, p, dev, None, debug_cost=True))
+        assert (a["plane_index"] >= 0).any()
+    # the split path against the oracle on its own (second family mostly wins below the horizon)
+    ctx.set_split("on")
+    ref, test, stats, _ = run_single(cfg, images, params=p, families=fam_sets[1], ctx=ctx)
+    assert_gates(stats, depth_frac_over_tol=0.01)
+    # batch and multi-resolution calls
+    planes = fsw.PlaneSet(fam_sets[0])
+    sets = [dev, [torch.from_numpy(im).cuda() for im in synth.render_frame(cfg, 0)]]
+    for s in range(2):
+        ctx.set_split("off")
+        single = oracle.compare.to_numpy(ctx.compute_depth(planes, p, sets[s], None))
+        ctx.set_split("on")
+        outs = ctx.compute_depth_batch(planes, p, sets, None)
+        torch.cuda.synchronize()
+        for key in keys:
+            assert np.array_equal(single[key], oracle.compare.to_numpy(outs[s])[key], equal_nan=True), (s, key)
+    pl, pc = fsw.PlaneSet(fam_sets[0]), fsw.PlaneSet(fam_sets[1])
+    pp = dict(p, window=3)
+    both(ctx, lambda: ctx.compute_depth_multires(pl, pc, pp, p, (40, 30, 70, 50), dev, None))
+    ctx.close()
+    # automatic mode at full size
+    cfg = synth.make_config(3)
+    _, _, ctx = gpu_objects(cfg)
+    planes = fsw.PlaneSet(cfg["families"])
+    dev = [torch.from_numpy(im).cuda() for im in synth.render_frame(cfg, 0)]
+    ctx.compute_depth(planes, cfg["params"], dev, None)
+    assert ctx.last_counters()["n_split_launches"] == 1
+    ctx.compute_depth_batch(planes, cfg["params"], [dev] * 8, None)
+    assert ctx.last_counters()["n_split_launches"] == 0
+    ctx.close()
+
+
 def test_bfloat16_and_float_footprints_agree_bitwise():
     """8-bit views are staged as bfloat16 footprints (exact for integers up to 256), float views as float footprints:
     the same integer-valued views given as uint8 and as float32 must produce bit-identical maps, and a call that
