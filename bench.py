@@ -30,7 +30,7 @@ FLOP_PER_EVAL = 70.0   # algorithmic FP32 work of one (pixel, pl
 N_STAGED = 32          # distinct frame sets resident on the device (the C5 stream length)
 METRIC = "plane-sweep cost evals/sec (pixel x plane x view)"
 # dram__bytes_read.sum + dram__bytes_write.sum of one sweep launch, from the committed ncu capture (profiles/)
-NCU_DRAM_BYTES_PER_LAUNCH = {("C5", 8): 157.3e6}
+NCU_DRAM_BYTES_PER_LAUNCH = {("C5", 8): 156.4e6}
 
 
 def parse_args():
@@ -337,9 +337,9 @@ def run_ours(args, rank, local_rank, world):
             "roofline": {"bound": "alu", "achieved": achieved, "peak": fp32_tflops, "unit": "TFLOP/s",
                          "frac": achieved / fp32_tflops if fp32_tflops else None,
                          "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get((args.workload, B)),
-                         "traffic_source": "profiles/r1_launches_c5.md (ncu --set full, dram bytes read + written by "
+                         "traffic_source": "profiles/r1_launches_c5_v6.md (ncu --set full, dram bytes read + written by "
                                            "one sweep launch)" if (args.workload, B) in NCU_DRAM_BYTES_PER_LAUNCH else None,
-                         "ncu_issue_active_pct": 65.1 if (args.workload, B) in NCU_DRAM_BYTES_PER_LAUNCH else None,
+                         "ncu_issue_active_pct": 65.6 if (args.workload, B) in NCU_DRAM_BYTES_PER_LAUNCH else None,
                          "frame_sets_per_launch": B, "evals_per_launch": evals_per_launch,
                          "kernel": "fsw::sweep_kernel<9,...>", "kernel_ms": sweep_ms_avg,
                          "flop_per_eval": FLOP_PER_EVAL,
