@@ -931,7 +931,8 @@ struct SweepInst {
     /* + 6: plane split (two work items per tile), built for the variants with one or two views only: the run-time
      * view loop with the split faulted on the device (misaligned address in the 9 x 9 instantiation) whenever the
      * halo plane, the descending half and the state exchange were all compiled in, and not with any one of them
-     * removed; fsw_api.cu does not split calls with more than two views until that is understood */
+     * removed, nor with ptxas at -O1; fsw_api.cu does not split calls with more than two views until that is
+     * understood */
     static constexpr int N_VARIANTS = NVT ? 12 : 6;
     static cudaError_t dispatch(const FswSweepArgs& args, int variant, int grid, cudaStream_t stream, bool prep) {
         switch (variant) {
