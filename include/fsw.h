@@ -251,6 +251,14 @@ int32_t fsw_compute_depth_multires_host(fsw_context* ctx, const fsw_planeset* pl
                                         const uint8_t* mask, size_t mask_pitch, const fsw_depth_out* out,
                                         void* cuda_stream);
 
+/* on != 0: the *_host calls of this context enqueue their host-to-device copies, kernels and device-to-host copies on
+ * the caller's stream and return WITHOUT synchronizing it.  The caller then owns the ordering: the host images, masks
+ * and outputs must stay untouched (and should be pinned, or the copies are not asynchronous) until the stream has
+ * reached the end of the call.  The staging buffers belong to the context, so calls issued on different streams need
+ * different contexts; with two contexts on two streams the copies of one frame-set batch overlap the sweep of the
+ * other (bench.py's end-to-end figure does exactly that).  Off by default.  Errors: FSW_E_INVALID_ARG (null). */
+int32_t fsw_context_set_host_async(fsw_context* ctx, int32_t on);
+
 /* Load balancing of calls with few frame sets (S0).  The sweep kernel runs one persistent CTA per SM over a queue of
  * (frame set, tile) items; a single 1280 x 1024 frame set has 176 live tiles for 148 SMs.  With the plane split every
  * tile becomes two work items that sweep one half of the planes each (the planes are independent

@@ -28,7 +28,7 @@ EXPORTS = (
     "fsw_planeset_table", "fsw_context_create", "fsw_context_destroy", "fsw_compute_depth",
     "fsw_compute_depth_multires", "fsw_compute_depth_host", "fsw_compute_depth_multires_host",
     "fsw_compute_depth_batch", "fsw_compute_depth_batch_host",
-    "fsw_context_set_timing", "fsw_context_set_split", "fsw_get_last_counters", "fsw_measure_fp32_peak", "fsw_filter_continuity",
+    "fsw_context_set_timing", "fsw_context_set_split", "fsw_context_set_host_async", "fsw_get_last_counters", "fsw_measure_fp32_peak", "fsw_filter_continuity",
 )
 
 
@@ -122,6 +122,7 @@ def load_library():
     L.fsw_compute_depth_multires_host.argtypes = multi
     L.fsw_context_set_timing.argtypes = [vp, i32]
     L.fsw_context_set_split.argtypes = [vp, i32]
+    L.fsw_context_set_host_async.argtypes = [vp, i32]
     L.fsw_get_last_counters.argtypes = [vp, P(CCounters)]
     L.fsw_measure_fp32_peak.argtypes = [i32, vp, P(ctypes.c_double), P(ctypes.c_double)]
     for name in EXPORTS:
@@ -432,6 +433,10 @@ class Context:
         _check(load_library().fsw_get_last_counters(self.handle, ctypes.byref(c)))
         return dict(n_eval=c.n_eval, n_raw_valid=c.n_raw_valid, n_valid=c.n_valid, n_launches=c.n_launches,
                     sweep_ms=c.sweep_ms, n_split_launches=c.n_split_launches)
+
+    def set_host_async(self, on=True):
+        """fsw_context_set_host_async: host=True calls return without synchronizing their stream."""
+        _check(load_library().fsw_context_set_host_async(self.handle, 1 if on else 0))
 
     def set_split(self, mode="auto"):
         """fsw_context_set_split: plane split of the tiles of calls with few frame sets ('auto', 'off', 'on')."""

@@ -120,6 +120,7 @@ struct fsw_context {
     DevBuf split_state;            /* plane split: [set][half][6][H][W] floats */
     DevBuf split_ticket;           /* plane split: one word per (set, tile), zero between launches */
     int32_t split_mode = FSW_SPLIT_AUTO;
+    bool host_async = false;       /* the *_host calls return without synchronizing their stream */
     int64_t last_split = 0;        /* sweep launches of the last call that split their tiles */
     std::vector<TileOrder*> orders;
     /* staging for the *_host calls: [set slot] */
@@ -935,7 +936,7 @@ static int32_t run_host(fsw_context* ctx, bool multires, const fsw_planeset* p0,
         if (out->plane_index) FSW_CUDA(cudaMemcpy2DAsync(out->plane_index, out->plane_index_pitch, o.plane_index, o.plane_index_pitch, (size_t)W * 2, H, cudaMemcpyDeviceToHost, stream));
         if (out->valid_reason) FSW_CUDA(cudaMemcpy2DAsync(out->valid_reason, out->valid_reason_pitch, o.valid_reason, o.valid_reason_pitch, (size_t)W, H, cudaMemcpyDeviceToHost, stream));
     }
-    FSW_CUDA(cudaStreamSynchronize(stream));
+    if (!ctx->host_async) FSW_CUDA(cudaStreamSynchronize(stream));
     return FSW_OK;
 }
 
@@ -990,6 +991,12 @@ int32_t fsw_filter_continuity(fsw_context* ctx, const float* depth_in, size_t de
     a.W = W; a.H = H; a.window = window;
     a.gamma = (double)gamma; a.delta = (double)delta;
     FSW_CUDA(fsw_launch_continuity(a, (cudaStream_t)cuda_stream));
+    return FSW_OK;
+}
+
+int32_t fsw_context_set_host_async(fsw_context* ctx, int32_t on) {
+    if (!ctx) return fail(FSW_E_INVALID_ARG, "fsw_context_set_host_async: null context");
+    ctx->host_async = on != 0;
     return FSW_OK;
 }
 

@@ -229,6 +229,37 @@ def test_host_call_equals_device_call_and_is_deterministic():
         assert np.array_equal(a[key], c[key], equal_nan=True), key
 
 
+def test_async_host_calls_on_two_streams():
+    """fsw_context_set_host_async: host calls that do not synchronize, issued alternately on two streams through two
+    contexts (bench.py's end-to-end arrangement), give the maps of the synchronous host call."""
+    import torch
+    import paper_1809_06132_b200 as fsw
+    cfg = _small_rig(W=150, H=77, n_views=2, fov=170.0)
+    rig = fsw.Rig(cfg["cams"], cfg["ref_index"])
+    planes = fsw.PlaneSet(cfg["families"])
+    ctxs = [fsw.Context(rig, 0), fsw.Context(rig, 0)]
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    sets = [[torch.from_numpy(im).pin_memory() for im in synth.render_frame(dict(cfg, scene=synth.scene_plane(2.0 + 0.5 * s, (0.5, 2.0), seed=40 + s)), 0)]
+            for s in range(6)]
+    masks = [torch.from_numpy(synth.make_mask(150, 77, 60 + s, n_rects=2)).pin_memory() for s in range(6)]
+    sync = [oracle.compare.to_numpy(ctxs[0].compute_depth(planes, cfg["params"], sets[s], masks[s], host=True)) for s in range(6)]
+    for c in ctxs:
+        c.set_host_async(True)
+    pinned = [{k: torch.empty((77, 150), dtype=t).pin_memory() for k, t in
+               (("depth", torch.float32), ("best_cost", torch.float32), ("second_cost", torch.float32),
+                ("plane_index", torch.int16), ("valid_reason", torch.uint8))} for _ in range(6)]
+    for b in range(3):  # batches of two frame sets, alternating contexts / streams
+        with torch.cuda.stream(streams[b % 2]):
+            ctxs[b % 2].compute_depth_batch(planes, cfg["params"], sets[2 * b:2 * b + 2], masks[2 * b:2 * b + 2], host=True,
+                                            outs=pinned[2 * b:2 * b + 2])
+    torch.cuda.synchronize()
+    for s in range(6):
+        for key in ("depth", "best_cost", "second_cost", "plane_index", "valid_reason"):
+            assert np.array_equal(sync[s][key], pinned[s][key].numpy(), equal_nan=True), (s, key)
+    for c in ctxs:
+        c.close()
+
+
 def test_multires_host_call_small():
     """S10 on a small rig: host-buffer call, crop not aligned to the tile grid, odd crop origin."""
     cfg = _small_rig(W=128, H=96, n_views=2, fov=170.0)
