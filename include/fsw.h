@@ -263,8 +263,9 @@ int32_t fsw_context_set_host_async(fsw_context* ctx, int32_t on);
  * (frame set, tile) items; a single 1280 x 1024 frame set has 176 live tiles for 148 SMs.  With the plane split every
  * tile becomes two work items that sweep one half of the planes each (the planes are independent
  * hypotheses) and merge their winner-take-all states; the maps are bit-identical to the unsplit ones.
- * FSW_SPLIT_AUTO (default): split when the live tiles of the call are fewer than three per SM; FSW_SPLIT_OFF: never;
- * FSW_SPLIT_ON: always.  Calls with fewer than two planes or more than two matching views are never split.  The context then owns 48 bytes of scratch per reference pixel
+ * FSW_SPLIT_AUTO (default): when the live tiles of the call are fewer than three per SM, the tiles beyond the last
+ * full wave of the grid are split (all of them if there is less than one wave); FSW_SPLIT_OFF: never;
+ * FSW_SPLIT_ON: every tile.  Calls with fewer than two planes or more than two matching views are never split.  The context then owns 48 bytes of scratch per reference pixel
  * and frame set of such a call.  Errors: FSW_E_INVALID_ARG for a null context or an unknown mode. */
 #define FSW_SPLIT_AUTO 0
 #define FSW_SPLIT_OFF 1

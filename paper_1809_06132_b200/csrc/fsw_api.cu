@@ -449,13 +449,17 @@ int32_t launch_sweep(fsw_context* ctx, FswSweepArgs& a, int w, cudaStream_t s) {
             }
             a.split = 1;
             a.split_k = kb;
+            /* As many full waves of whole tiles as the live tiles fill (the heaviest come first in the queue), the
+             * rest in halves: 148 whole + 28 split tiles for one 1280 x 1024 frame set.  FSW_SPLIT_ON halves all. */
+            const long long live_items = live * a.n_sets;
+            a.split_whole = (ctx->split_mode == FSW_SPLIT_ON || live_items < slots) ? 0 : (int32_t)(slots * (live_items / slots));
             a.split_adjacent = fa == fb ? 1 : 0;
             a.split_state = (float*)ctx->split_state.p;
             a.split_ticket = (unsigned int*)ctx->split_ticket.p;
         }
     }
     ctx->last_split += a.split;
-    const long long items = (long long)a.n_tiles * a.n_sets * (a.split ? 2 : 1);
+    const long long items = a.split ? 2LL * a.n_tiles * a.n_sets - a.split_whole : (long long)a.n_tiles * a.n_sets;
     const int grid = (int)(items < slots ? items : slots);
     const int var = pick_variant(a, a.foot_f16) + (a.split ? 6 : 0);
     cudaError_t e = cudaErrorInvalidValue;

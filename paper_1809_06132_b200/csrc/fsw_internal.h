@@ -110,11 +110,12 @@ struct FswSweepArgs {
     int32_t n_tiles_x, n_tiles;
     unsigned int* queue; /* zero before the launch; CTAs claim items beyond gridDim.x from it */
     /* plane split (single frame sets do not fill the persistent grid: 176 live tiles of a 1280 x 1024 frame for 148
-     * CTAs): with split = 1 every (set, tile) is two work items, item half 0 sweeps the planes [0, split_k) in
+     * CTAs): with split = 1 a (set, tile) slot is two work items, item half 0 sweeps the planes [0, split_k) in
      * ascending order, half 1 the planes [split_k, P) in descending order; the half that finishes first leaves its
      * winner-take-all state in split_state ([n_sets][6][H][W] floats), the other one merges it into its registers
      * and runs S8-S12.  split_ticket: one word per (set, tile), zero before and after the launch. */
     int32_t split, split_k;
+    int32_t split_whole;    /* the first split_whole (tile, set) slots of the queue are swept whole, the rest in halves */
     int32_t split_adjacent; /* planes split_k - 1 and split_k belong to the same family */
     float* split_state;
     unsigned int* split_ticket;

@@ -469,7 +469,8 @@ __global__ void __launch_bounds__(Geo<WIN>::NT, 1) sweep_kernel(const __grid_con
     /* [TY][TX]: reference-side window statistics of every output: ((sum a')/N, sum a'^2 - (sum a')^2/N) */
     float2* const a_stat = reinterpret_cast<float2*>(hs + 4 * G::HPLANE) + (grp * RPT) * TX + col;
     const int W = args.ref.W, H = args.ref.H;
-    const int n_items = args.n_tiles * args.n_sets * (SPLIT ? 2 : 1);
+    /* split launches: the first split_whole (tile, set) slots are swept whole, every later one as two halves */
+    const int n_items = SPLIT ? 2 * args.n_tiles * args.n_sets - args.split_whole : args.n_tiles * args.n_sets;
     const int n_views = NVT ? NVT : args.n_views;
 
     /* this lane's halo pixels: slot i is element lane + 32 i of the warp's R x SB block of the sample planes; in the
@@ -488,14 +489,16 @@ __global__ void __launch_bounds__(Geo<WIN>::NT, 1) sweep_kernel(const __grid_con
 
     unsigned item = blockIdx.x;
     while (item < (unsigned)n_items) {
-        /* plane split: item = 2 * (tile slot) + half; own planes [k_lo, k_hi), visited downwards in half 1 */
-        const int half = SPLIT ? (int)(item & 1u) : 0;
-        const unsigned titem = SPLIT ? item >> 1 : item;
-        const bool desc = SPLIT && half != 0;
+        /* plane split: the slots beyond split_whole are two items each, half 0 and half 1; own planes [k_lo, k_hi),
+         * visited downwards in half 1 */
+        const bool halved = SPLIT && item >= (unsigned)args.split_whole;
+        const int half = halved ? (int)((item - (unsigned)args.split_whole) & 1u) : 0;
+        const unsigned titem = halved ? (unsigned)args.split_whole + ((item - (unsigned)args.split_whole) >> 1) : item;
+        const bool desc = halved && half != 0;
         const int dir = desc ? -1 : 1;
-        const int k_lo = desc ? args.split_k : 0, k_hi = (SPLIT && !half) ? args.split_k : args.n_planes;
+        const int k_lo = desc ? args.split_k : 0, k_hi = (halved && !half) ? args.split_k : args.n_planes;
         /* the plane across the cut, evaluated only as the parabola neighbour of a winner next to the cut */
-        const int k_halo = (SPLIT && args.split_adjacent) ? (half ? args.split_k - 1 : args.split_k) : -1;
+        const int k_halo = (halved && args.split_adjacent) ? (half ? args.split_k - 1 : args.split_k) : -1;
         const int set = (int)(titem % (unsigned)args.n_sets);
         const int tile = args.tile_order[titem / (unsigned)args.n_sets];
         const FswSetPtrs& S = args.n_sets > 1 ? args.sets[set] : args.set0;
@@ -781,7 +784,7 @@ __global__ void __launch_bounds__(Geo<WIN>::NT, 1) sweep_kernel(const __grid_con
 #pragma unroll
             for (int i = 0; i < RPT; ++i) st[i].swap_neighbours();
         }
-        if (SPLIT) {
+        if (halved) {
             if (!tile_active) {
                 do_epilogue = half == 0; /* nothing was swept: one half writes the invalid / upsampled outputs */
             } else {

@@ -385,8 +385,15 @@ def test_plane_split_is_bit_identical_to_the_unsplit_sweep():
     _, _, ctx = gpu_objects(cfg)
     planes = fsw.PlaneSet(cfg["families"])
     dev = [torch.from_numpy(im).cuda() for im in synth.render_frame(cfg, 0)]
-    ctx.compute_depth(planes, cfg["params"], dev, None)
-    assert ctx.last_counters()["n_split_launches"] == 1
+    res = {}
+    for mode in ("off", "auto", "on"):  # auto: 148 whole tiles + the other live tiles in halves; on: every tile in halves
+        ctx.set_split(mode)
+        res[mode] = oracle.compare.to_numpy(ctx.compute_depth(planes, cfg["params"], dev, None))
+        assert ctx.last_counters()["n_split_launches"] == (0 if mode == "off" else 1)
+    for mode in ("auto", "on"):
+        for key in keys:
+            assert np.array_equal(res["off"][key], res[mode][key], equal_nan=True), (mode, key)
+    ctx.set_split("auto")
     ctx.compute_depth_batch(planes, cfg["params"], [dev] * 8, None)
     assert ctx.last_counters()["n_split_launches"] == 0
     ctx.close()
