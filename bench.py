@@ -266,7 +266,6 @@ def run_ours(args, rank, local_rank, world):
         step(f)
         c = ctx.last_counters()
         n_eval_step.append(c["n_eval"])
-        launches_per_step = c["n_launches"]
     sampler = ClockSampler(physical_gpu_index(local_rank))
     stream = torch.cuda.current_stream()
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -279,6 +278,7 @@ def run_ours(args, rank, local_rank, world):
     sampler.stop_flag = True
     barrier()
     ms_total = ev0.elapsed_time(ev1)
+    launches_per_step = ctx.last_counters()["n_launches"]  # kernels of one call of the timed loop (B frame sets)
     n_calls = (args.steps + B - 1) // B
     launches = launches_per_step * n_calls
     evals_total = float(sum(n_eval_step[i % len(n_eval_step)] for i in range(args.steps)))

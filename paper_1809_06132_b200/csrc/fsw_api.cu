@@ -104,8 +104,9 @@ struct TileOrder {
     DevBuf dev;
 };
 
-/* words of the control block: [0] work queue of the sweep kernel, [2..9] four 64-bit counters */
+/* words of the control block: [0], [1] work queues of the sweep launches, [2..9] four 64-bit counters */
 #define FSW_CTRL_WORDS 10
+#define FSW_QUEUE_WORDS 2 /* [0] queue of the (first) sweep launch, [1] queue of the launch of the halved tiles */
 
 struct fsw_context {
     fsw_rig rig;
@@ -121,6 +122,9 @@ struct fsw_context {
     DevBuf split_ticket;           /* plane split: one word per (set, tile), zero between launches */
     int32_t split_mode = FSW_SPLIT_AUTO;
     bool host_async = false;       /* the *_host calls return without synchronizing their stream */
+    /* second launch of a split call (the halved tiles), ordered against the caller's stream by two events */
+    cudaStream_t aux_stream = nullptr;
+    cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
     int64_t last_split = 0;        /* sweep launches of the last call that split their tiles */
     std::vector<TileOrder*> orders;
     /* staging for the *_host calls: [set slot] */
@@ -459,18 +463,51 @@ int32_t launch_sweep(fsw_context* ctx, FswSweepArgs& a, int w, cudaStream_t s) {
         }
     }
     ctx->last_split += a.split;
-    const long long items = a.split ? 2LL * a.n_tiles * a.n_sets - a.split_whole : (long long)a.n_tiles * a.n_sets;
-    const int grid = (int)(items < slots ? items : slots);
-    const int var = pick_variant(a, a.foot_f16) + (a.split ? 6 : 0);
-    cudaError_t e = cudaErrorInvalidValue;
-    switch (w) {
-        case 3: e = fsw_launch_sweep_w3(a, var, grid, s); break;
-        case 5: e = fsw_launch_sweep_w5(a, var, grid, s); break;
-        case 7: e = fsw_launch_sweep_w7(a, var, grid, s); break;
-        case 9: e = fsw_launch_sweep_w9(a, var, grid, s); break;
-        case 11: e = fsw_launch_sweep_w11(a, var, grid, s); break;
-        case 13: e = fsw_launch_sweep_w13(a, var, grid, s); break;
-        case 15: e = fsw_launch_sweep_w15(a, var, grid, s); break;
+    const int total_slots = a.n_tiles * a.n_sets;
+    auto launch_one = [&](const FswSweepArgs& la, cudaStream_t ls) -> cudaError_t {
+        const long long items = la.split ? 2LL * la.slot_count - la.split_whole : (long long)la.slot_count;
+        const int grid = (int)(items < slots ? items : slots);
+        const int var = pick_variant(la, la.foot_f16) + (la.split ? 6 : 0);
+        switch (w) {
+            case 3: return fsw_launch_sweep_w3(la, var, grid, ls);
+            case 5: return fsw_launch_sweep_w5(la, var, grid, ls);
+            case 7: return fsw_launch_sweep_w7(la, var, grid, ls);
+            case 9: return fsw_launch_sweep_w9(la, var, grid, ls);
+            case 11: return fsw_launch_sweep_w11(la, var, grid, ls);
+            case 13: return fsw_launch_sweep_w13(la, var, grid, ls);
+            case 15: return fsw_launch_sweep_w15(la, var, grid, ls);
+        }
+        return cudaErrorInvalidValue;
+    };
+    a.slot_first = 0;
+    a.slot_count = total_slots;
+    cudaError_t e;
+    if (a.split && a.split_whole > 0) {
+        /* Two launches: the whole tiles (the first full waves of the queue) in the unsplit instantiation on the
+         * caller's stream, the halved tiles in the split instantiation on a low-priority stream of the context that
+         * is forked from and joined to the caller's stream by events; its CTAs take the SMs the first launch frees. */
+        if (!ctx->aux_stream) {
+            int lo = 0, hi = 0;
+            FSW_CUDA(cudaDeviceGetStreamPriorityRange(&lo, &hi));
+            FSW_CUDA(cudaStreamCreateWithPriority(&ctx->aux_stream, cudaStreamNonBlocking, lo));
+            FSW_CUDA(cudaEventCreateWithFlags(&ctx->ev_fork, cudaEventDisableTiming));
+            FSW_CUDA(cudaEventCreateWithFlags(&ctx->ev_join, cudaEventDisableTiming));
+        }
+        FswSweepArgs whole = a, halves = a;
+        whole.split = 0; whole.split_whole = 0; whole.slot_first = 0; whole.slot_count = a.split_whole;
+        halves.split_whole = 0; halves.slot_first = a.split_whole; halves.slot_count = total_slots - a.split_whole;
+        halves.queue = ctx->queue() + 1;
+        FSW_CUDA(cudaEventRecord(ctx->ev_fork, s));
+        e = launch_one(whole, s);
+        if (e == cudaSuccess) {
+            FSW_CUDA(cudaStreamWaitEvent(ctx->aux_stream, ctx->ev_fork, 0));
+            e = launch_one(halves, ctx->aux_stream);
+            FSW_CUDA(cudaEventRecord(ctx->ev_join, ctx->aux_stream));
+            FSW_CUDA(cudaStreamWaitEvent(s, ctx->ev_join, 0));
+            ctx->last_launches++;
+        }
+    } else {
+        e = launch_one(a, s);
     }
     if (e != cudaSuccess) return cuda_fail(e, "sweep kernel launch");
     ctx->last_launches++;
@@ -504,7 +541,7 @@ int32_t stage_views(fsw_context* ctx, const fsw_image* images, int n_sets, bool 
             if (pk.n == 0) return FSW_OK;
             if (first) {
                 pk.words_to_zero = (unsigned int*)ctx->ctrl.p;
-                pk.n_words_to_zero = zero_counters ? FSW_CTRL_WORDS : 1;
+                pk.n_words_to_zero = zero_counters ? FSW_CTRL_WORDS : FSW_QUEUE_WORDS;
                 first = false;
             } else {
                 pk.words_to_zero = nullptr;
@@ -544,7 +581,7 @@ int32_t stage_views(fsw_context* ctx, const fsw_image* images, int n_sets, bool 
         if (rc != FSW_OK) return rc;
     }
     if (first) /* cannot happen (a rig has at least one view), but never start a sweep with a dirty queue */
-        FSW_CUDA(cudaMemsetAsync(ctx->ctrl.p, 0, (zero_counters ? FSW_CTRL_WORDS : 1) * sizeof(unsigned int), stream));
+        FSW_CUDA(cudaMemsetAsync(ctx->ctrl.p, 0, (zero_counters ? FSW_CTRL_WORDS : FSW_QUEUE_WORDS) * sizeof(unsigned int), stream));
     return FSW_OK;
 }
 
@@ -717,6 +754,7 @@ int32_t fsw_context_destroy(fsw_context* ctx) {
     ctx->lo_depth.release(); ctx->lo_c1.release(); ctx->lo_c2.release(); ctx->lo_k.release();
     ctx->ctrl.release(); ctx->sets_dev.release();
     ctx->split_state.release(); ctx->split_ticket.release();
+    if (ctx->aux_stream) { cudaStreamDestroy(ctx->aux_stream); cudaEventDestroy(ctx->ev_fork); cudaEventDestroy(ctx->ev_join); }
     for (TileOrder* t : ctx->orders) {
         t->dev.release();
         delete t;
