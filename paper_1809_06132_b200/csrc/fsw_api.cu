@@ -457,6 +457,7 @@ int32_t launch_sweep(fsw_context* ctx, FswSweepArgs& a, int w, cudaStream_t s) {
              * rest in halves: 148 whole + 28 split tiles for one 1280 x 1024 frame set.  FSW_SPLIT_ON halves all. */
             const long long live_items = live * a.n_sets;
             a.split_whole = (ctx->split_mode == FSW_SPLIT_ON || live_items < slots) ? 0 : (int32_t)(slots * (live_items / slots));
+            a.split_whole -= a.split_whole % a.n_sets; /* whole tiles of every set: the first launch sees fewer tiles */
             a.split_adjacent = fa == fb ? 1 : 0;
             a.split_state = (float*)ctx->split_state.p;
             a.split_ticket = (unsigned int*)ctx->split_ticket.p;
@@ -465,7 +466,7 @@ int32_t launch_sweep(fsw_context* ctx, FswSweepArgs& a, int w, cudaStream_t s) {
     ctx->last_split += a.split;
     const int total_slots = a.n_tiles * a.n_sets;
     auto launch_one = [&](const FswSweepArgs& la, cudaStream_t ls) -> cudaError_t {
-        const long long items = la.split ? 2LL * la.slot_count - la.split_whole : (long long)la.slot_count;
+        const long long items = la.split ? 2LL * la.slot_count - la.split_whole : (long long)la.n_tiles * la.n_sets;
         const int grid = (int)(items < slots ? items : slots);
         const int var = pick_variant(la, la.foot_f16) + (la.split ? 6 : 0);
         switch (w) {
@@ -494,7 +495,8 @@ int32_t launch_sweep(fsw_context* ctx, FswSweepArgs& a, int w, cudaStream_t s) {
             FSW_CUDA(cudaEventCreateWithFlags(&ctx->ev_join, cudaEventDisableTiming));
         }
         FswSweepArgs whole = a, halves = a;
-        whole.split = 0; whole.split_whole = 0; whole.slot_first = 0; whole.slot_count = a.split_whole;
+        whole.split = 0; whole.split_whole = 0;
+        whole.n_tiles = a.split_whole / a.n_sets; /* the unsplit kernel sweeps the first n_tiles * n_sets slots */
         halves.split_whole = 0; halves.slot_first = a.split_whole; halves.slot_count = total_slots - a.split_whole;
         halves.queue = ctx->queue() + 1;
         FSW_CUDA(cudaEventRecord(ctx->ev_fork, s));

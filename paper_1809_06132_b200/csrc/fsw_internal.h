@@ -108,7 +108,7 @@ struct FswSweepArgs {
     /* work queue: items = n_sets * n_tiles, item i -> set i % n_sets, tile tile_order[i / n_sets] */
     const int32_t* tile_order; /* device, n_tiles entries: tile index ty * n_tiles_x + tx, heaviest first */
     int32_t n_tiles_x, n_tiles;
-    int32_t slot_first, slot_count; /* the (tile, set) slots of the queue order this launch covers (all: 0, n_tiles * n_sets) */
+    int32_t slot_first, slot_count; /* split launches: the (tile, set) slots of the queue order the launch covers */
     unsigned int* queue; /* zero before the launch; CTAs claim items beyond gridDim.x from it */
     /* plane split (single frame sets do not fill the persistent grid: 176 live tiles of a 1280 x 1024 frame for 148
      * CTAs): with split = 1 a (set, tile) slot is two work items, item half 0 sweeps the planes [0, split_k) in

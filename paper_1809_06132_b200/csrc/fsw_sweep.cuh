@@ -470,8 +470,9 @@ __global__ void __launch_bounds__(Geo<WIN>::NT, 1) sweep_kernel(const __grid_con
     float2* const a_stat = reinterpret_cast<float2*>(hs + 4 * G::HPLANE) + (grp * RPT) * TX + col;
     const int W = args.ref.W, H = args.ref.H;
     /* split launches: the first split_whole (tile, set) slots are swept whole, every later one as two halves */
-    /* this launch covers the (tile, set) slots slot_first .. slot_first + slot_count - 1 of the queue order */
-    const int n_items = SPLIT ? 2 * args.slot_count - args.split_whole : args.slot_count;
+    /* a split launch covers the (tile, set) slots slot_first .. slot_first + slot_count - 1 of the queue order, an
+     * unsplit one the first n_tiles * n_sets */
+    const int n_items = SPLIT ? 2 * args.slot_count - args.split_whole : args.n_tiles * args.n_sets;
     const int n_views = NVT ? NVT : args.n_views;
 
     /* this lane's halo pixels: slot i is element lane + 32 i of the warp's R x SB block of the sample planes; in the
@@ -494,7 +495,7 @@ __global__ void __launch_bounds__(Geo<WIN>::NT, 1) sweep_kernel(const __grid_con
          * visited downwards in half 1 */
         const bool halved = SPLIT && item >= (unsigned)args.split_whole;
         const int half = halved ? (int)((item - (unsigned)args.split_whole) & 1u) : 0;
-        const unsigned titem = (unsigned)args.slot_first +
+        const unsigned titem = !SPLIT ? item : (unsigned)args.slot_first +
                                (halved ? (unsigned)args.split_whole + ((item - (unsigned)args.split_whole) >> 1) : item);
         const bool desc = halved && half != 0;
         const int dir = desc ? -1 : 1;
