@@ -198,7 +198,7 @@ int32_t fsw_planeset_table(const fsw_planeset* ps, double* s, double* d, int32_t
  * queue, counters).  Scratch is allocated lazily and reused, so one context serves one stream at a time.  All work of
  * a call is ordered on the stream given to it: whatever follows the call on that stream sees its results.  (A split
  * call, fsw_context_set_split, runs its second sweep launch on a low-priority stream of the context that is forked
- * from and joined to the caller's stream by events; this is compatible with stream capture.) */
+ * from and joined to the caller's stream by events.) */
 int32_t fsw_context_create(const fsw_rig* rig, int32_t cuda_device, fsw_context** out);
 int32_t fsw_context_destroy(fsw_context* ctx);
 
