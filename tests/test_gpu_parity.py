@@ -399,6 +399,31 @@ def test_plane_split_is_bit_identical_to_the_unsplit_sweep():
     ctx.close()
 
 
+@pytest.mark.parametrize("window", [7, 11])
+def test_plane_split_two_launches_other_windows(window):
+    """An image with more live tiles than SMs and a window other than 9 x 9 (other tile geometry): the automatic mode
+    sweeps the first full wave whole and the rest in halves, in two launches, and gives the unsplit maps bit for bit."""
+    import torch
+    import paper_1809_06132_b200 as fsw
+    cfg = _small_rig(W=1216, H=808, n_views=2, fov=170.0)
+    _, _, ctx = gpu_objects(cfg)
+    planes = fsw.PlaneSet([synth.family((0, 0, 1), 9, 0.8, 30.0, "inverse"), synth.family((0, 1, 0), 4, 0.4, 1.6, "linear")])
+    dev = [torch.from_numpy(im).cuda() for im in synth.render_frame(cfg, 0)]
+    p = dict(cfg["params"], window=window, filters=3, alpha_upper=0.4, alpha_lower=0.4, beta=1.05, horizon_row=400)
+    res = {}
+    for mode in ("off", "auto"):
+        ctx.set_split(mode)
+        res[mode] = oracle.compare.to_numpy(ctx.compute_depth(planes, p, dev, None))
+        c = ctx.last_counters()
+        assert (c["n_split_launches"], c["n_launches"]) == ((0, 2) if mode == "off" else (1, 3)), c
+        res[mode + "_n_eval"] = c["n_eval"]
+    assert res["off_n_eval"] == res["auto_n_eval"] > 0
+    for key in ("depth", "best_cost", "second_cost", "plane_index", "valid_reason"):
+        assert np.array_equal(res["off"][key], res["auto"][key], equal_nan=True), key
+    assert (res["off"]["plane_index"] >= 0).sum() > 100000
+    ctx.close()
+
+
 def test_bfloat16_and_float_footprints_agree_bitwise():
     """8-bit views are staged as bfloat16 footprints (exact for integers up to 256), float views as float footprints:
     the same integer-valued views given as uint8 and as float32 must produce bit-identical maps, and a call that
