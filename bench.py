@@ -335,7 +335,8 @@ def run_ours(args, rank, local_rank, world):
     (ms_total, ms_e2e), (evals_all,) = shard.reduce_timing([ms_total, ms_e2e], [evals_total], dev)
 
     if rank == 0:
-        fp32_tflops, _ = fsw.measure_fp32_peak(local_rank)
+        from paper_1809_06132_b200.probe import measure_fp32_peak
+        fp32_tflops, _ = measure_fp32_peak(local_rank)
         value = evals_all / (ms_total * 1e-3)
         e2e_value = evals_all / (ms_e2e * 1e-3)
         achieved = evals_per_launch * FLOP_PER_EVAL / (sweep_ms_avg * 1e-3) / 1e12

@@ -196,9 +196,9 @@ int32_t fsw_planeset_table(const fsw_planeset* ps, double* s, double* d, int32_t
 /* ---- context (needs a CUDA device) ---------------------------------------- */
 /* Owns device-side scratch (footprint images of the views, half-resolution images and maps, tile schedule, work
  * queue, counters).  Scratch is allocated lazily and reused, so one context serves one stream at a time.  All work of
- * a call is ordered on the stream given to it: whatever follows the call on that stream sees its results.  (A split
- * call, fsw_context_set_split, runs its second sweep launch on a low-priority stream of the context that is forked
- * from and joined to the caller's stream by events.) */
+ * a call is ordered on the stream given to it: whatever follows the call on that stream sees its results.  The
+ * library launches on no other stream ("no hidden streams") unless the caller opts in with
+ * fsw_context_set_split(ctx, FSW_SPLIT_AUTO_TWO_STREAMS). */
 int32_t fsw_context_create(const fsw_rig* rig, int32_t cuda_device, fsw_context** out);
 int32_t fsw_context_destroy(fsw_context* ctx);
 
@@ -266,30 +266,43 @@ int32_t fsw_context_set_host_async(fsw_context* ctx, int32_t on);
  * tile becomes two work items that sweep one half of the planes each (the planes are independent
  * hypotheses) and merge their winner-take-all states; the maps are bit-identical to the unsplit ones.
  * FSW_SPLIT_AUTO (default): when the live tiles of the call are fewer than three per SM, the tiles beyond the last
- * full wave of the grid are split (all of them if there is less than one wave); FSW_SPLIT_OFF: never;
- * FSW_SPLIT_ON: every tile.  Calls with fewer than two planes or more than two matching views are never split.  The context then owns 48 bytes of scratch per reference pixel
- * and frame set of such a call.  Errors: FSW_E_INVALID_ARG for a null context or an unknown mode. */
+ * full wave of the grid are split (all of them if there is less than one wave), in ONE launch on the caller's stream;
+ * FSW_SPLIT_OFF: never; FSW_SPLIT_ON: every tile.
+ * FSW_SPLIT_AUTO_TWO_STREAMS (opt-in, the only mode in which the library uses a stream of its own): as AUTO, but the
+ * whole tiles and the halved tiles go into two launches, the second one on a low-priority stream the context creates,
+ * forked from and joined to the caller's stream by two events, so that its thread blocks take the SMs the first
+ * launch frees (about 5 % less latency for a single 1280 x 1024 frame set).  To the caller the call is still ordered
+ * on its stream; under stream capture the fork / join events make the second stream part of the captured graph, but a
+ * caller that confines its stream to an SM partition (green context) should not use this mode: the context's stream is
+ * created on the device's primary context.
+ * Calls with fewer than two planes are never split.  The context owns 48 bytes of scratch per reference pixel and
+ * frame set of a split call.  Errors: FSW_E_INVALID_ARG for a null context or an unknown mode. */
 #define FSW_SPLIT_AUTO 0
 #define FSW_SPLIT_OFF 1
 #define FSW_SPLIT_ON 2
+#define FSW_SPLIT_AUTO_TWO_STREAMS 3
 int32_t fsw_context_set_split(fsw_context* ctx, int32_t mode);
 
-/* on != 0: every following compute call brackets its sweep kernel launches (the dominant kernels, S1-S12) with a
- * pair of CUDA events on the call's stream so that fsw_get_last_counters can report their device time.  Off by
- * default (two event records per call). */
+/* Part of the statistics call below (SURVEY.md 8(b) "stats ... for benches only"): on != 0 makes every following
+ * compute call bracket its sweep kernel launches (the dominant kernels, S1-S12) with a pair of CUDA events on the
+ * call's stream so that fsw_get_last_counters can report their device time (the roofline record of bench.py needs the
+ * duration of that kernel alone, measured on the stream it is launched on).  Off by default (two event records per
+ * call); it changes no result. */
 int32_t fsw_context_set_timing(fsw_context* ctx, int32_t on);
 
 /* Counters of the most recent compute call on this context.  Synchronizes the stream that call used. */
 int32_t fsw_get_last_counters(fsw_context* ctx, fsw_counters* out);
 
 /* ---- local depth-continuity filter ------------------------------------------ */
-/* The third filter of PAPER.md:99 ("we compare its depth value against the depths of its neighboring pixels in a local
- * window. If the difference is smaller than a threshold gamma, we will consider the neighboring pixels to be consistent
- * with the central pixel. If the ratio of the consistent pixels in the local window is smaller than delta, we will
- * consider the center pixel to have inaccurate depth"; gamma = 0.5 m, delta = 0.3), followed by the mask.
+/* The third filter of PAPER.md:99: a pixel's depth is held against the depths around it in a local window; a
+ * neighbour whose depth differs by less than gamma counts as consistent with the centre, and the centre is rejected
+ * when the consistent share of the window falls below delta (the paper states gamma = 0.5 m and delta = 0.3).  The
+ * mask follows.
  * Reading Q25: window x window neighbourhood (odd, 3..FSW_MAX_WINDOW; SPEC.md proposes 5) without the
  * centre; a neighbour is consistent iff it is valid (depth > 0), inside the image and |d_n - d_c| < gamma (compared in
- * double precision); the centre is invalidated iff consistent / (window^2 - 1) < delta.  Only depth_in is read (never a
+ * double precision); the centre is invalidated iff consistent / (window^2 - 1) < delta, decided in double precision
+ * with gamma and delta as given (they are doubles in this ABI: delta = 0.3 with a 9 x 9 window keeps a centre with
+ * exactly 24 consistent neighbours of 80, which a float 0.3f > 0.3 would reject).  Only depth_in is read (never a
  * partially filtered state), so depth_out must not overlap depth_in.
  * depth_in / depth_out: device, float32, reference-camera size of the context's rig, pitches in BYTES, 0.0f = invalid.
  * Call fsw_compute_depth* WITHOUT a mask and pass the mask here (nullable): the mask comes after the filters.
@@ -298,14 +311,9 @@ int32_t fsw_get_last_counters(fsw_context* ctx, fsw_counters* out);
  * Errors: FSW_E_INVALID_ARG (null pointers, even / out-of-range window, gamma <= 0, delta outside [0,1], pitches too
  * small, overlapping depth buffers), FSW_E_CUDA. */
 int32_t fsw_filter_continuity(fsw_context* ctx, const float* depth_in, size_t depth_in_pitch, int32_t window,
-                              float gamma, float delta, const uint8_t* mask, size_t mask_pitch,
+                              double gamma, double delta, const uint8_t* mask, size_t mask_pitch,
                               float* depth_out, size_t depth_out_pitch, uint8_t* reason_out, size_t reason_pitch,
                               void* cuda_stream);
-
-/* ---- measurement helper ---------------------------------------------------- */
-/* Runs a dependent-FFMA-chain kernel on `cuda_stream` and reports the FP32 throughput it reached (TFLOP/s, counting
- * an FMA as 2) and the kernel time.  Used by bench.py for the "alu" roofline denominator. Synchronizes. */
-int32_t fsw_measure_fp32_peak(int32_t cuda_device, void* cuda_stream, double* tflops, double* ms);
 
 #ifdef __cplusplus
 }

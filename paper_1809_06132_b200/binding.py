@@ -28,7 +28,7 @@ EXPORTS = (
     "fsw_planeset_table", "fsw_context_create", "fsw_context_destroy", "fsw_compute_depth",
     "fsw_compute_depth_multires", "fsw_compute_depth_host", "fsw_compute_depth_multires_host",
     "fsw_compute_depth_batch", "fsw_compute_depth_batch_host",
-    "fsw_context_set_timing", "fsw_context_set_split", "fsw_context_set_host_async", "fsw_get_last_counters", "fsw_measure_fp32_peak", "fsw_filter_continuity",
+    "fsw_context_set_timing", "fsw_context_set_split", "fsw_context_set_host_async", "fsw_get_last_counters", "fsw_filter_continuity",
 )
 
 
@@ -124,7 +124,6 @@ def load_library():
     L.fsw_context_set_split.argtypes = [vp, i32]
     L.fsw_context_set_host_async.argtypes = [vp, i32]
     L.fsw_get_last_counters.argtypes = [vp, P(CCounters)]
-    L.fsw_measure_fp32_peak.argtypes = [i32, vp, P(ctypes.c_double), P(ctypes.c_double)]
     for name in EXPORTS:
         if name != "fsw_last_error":
             getattr(L, name).restype = i32
@@ -293,20 +292,25 @@ class Context:
 
     def _outputs(self, host, want, out=None):
         torch = _torch()
+        W, H = self.rig.sizes[self.rig.ref_index]
+        spec = dict(depth=torch.float32, best_cost=torch.float32, second_cost=torch.float32, plane_index=torch.int16,
+                    valid_reason=torch.uint8)
         if out is not None:  # caller-owned output tensors (e.g. pinned host buffers reused across calls)
             c = CDepthOut()
             c.struct_size = ctypes.sizeof(CDepthOut)
-            for name in ("depth", "best_cost", "second_cost", "plane_index", "valid_reason"):
+            assert out.get("depth") is not None, "the depth map is required"
+            for name, dt in spec.items():
                 t = out.get(name)
                 if t is not None:
-                    assert t.is_cuda != host and t.stride(1) == 1
+                    # fsw.h sees pointers and pitches only: type, shape and device are checked here
+                    assert t.dtype == dt, "%s must be %s" % (name, dt)
+                    assert tuple(t.shape) == (H, W) and t.stride(1) == 1, "%s must be a row-major (H, W) map" % name
+                    assert t.is_cuda != host, "%s is on the wrong side (host=%s)" % (name, host)
+                    assert host or t.device.index == self.device, "%s is on another GPU than the context" % name
                     setattr(c, name, t.data_ptr())
                     setattr(c, name + "_pitch", t.stride(0) * t.element_size())
             return c, dict(out)
-        W, H = self.rig.sizes[self.rig.ref_index]
         kw = dict(device="cpu", pin_memory=True) if host else dict(device="cuda:%d" % self.device)
-        spec = dict(depth=torch.float32, best_cost=torch.float32, second_cost=torch.float32, plane_index=torch.int16,
-                    valid_reason=torch.uint8)
         out, c = {}, CDepthOut()
         c.struct_size = ctypes.sizeof(CDepthOut)
         for name, dt in spec.items():
@@ -327,7 +331,7 @@ class Context:
             assert m.shape == (H, W)
             return m.ctypes.data, m.strides[0], m
         assert mask.dtype == torch.uint8 and tuple(mask.shape) == (H, W) and mask.stride(1) == 1
-        assert mask.is_cuda != host
+        assert mask.is_cuda != host and (host or mask.device.index == self.device)
         return mask.data_ptr(), mask.stride(0), mask
 
     ALL = ("best_cost", "second_cost", "plane_index", "valid_reason")
@@ -413,13 +417,14 @@ class Context:
         Returns dict(depth=..., valid_reason=...) of new device tensors."""
         torch = _torch()
         W, H = self.rig.sizes[self.rig.ref_index]
-        assert depth.is_cuda and depth.dtype == torch.float32 and tuple(depth.shape) == (H, W) and depth.stride(1) == 1
+        assert depth.is_cuda and depth.device.index == self.device, "depth must live on the context's GPU"
+        assert depth.dtype == torch.float32 and tuple(depth.shape) == (H, W) and depth.stride(1) == 1
         out = torch.empty((H, W), dtype=torch.float32, device=depth.device)
         reason = torch.empty((H, W), dtype=torch.uint8, device=depth.device) if want_reason else None
         mptr, mpitch, mkeep = self._mask(mask, False)
         stream = torch.cuda.current_stream(self.device).cuda_stream
         fn = load_library().fsw_filter_continuity
-        fn.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_size_t, ctypes.c_int32, ctypes.c_float, ctypes.c_float,
+        fn.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_size_t, ctypes.c_int32, ctypes.c_double, ctypes.c_double,
                        ctypes.c_void_p, ctypes.c_size_t, ctypes.c_void_p, ctypes.c_size_t, ctypes.c_void_p,
                        ctypes.c_size_t, ctypes.c_void_p]
         _check(fn(self.handle, depth.data_ptr(), depth.stride(0) * 4, int(window), float(gamma), float(delta),
@@ -439,18 +444,10 @@ class Context:
         _check(load_library().fsw_context_set_host_async(self.handle, 1 if on else 0))
 
     def set_split(self, mode="auto"):
-        """fsw_context_set_split: plane split of the tiles of calls with few frame sets ('auto', 'off', 'on')."""
-        _check(load_library().fsw_context_set_split(self.handle, {"auto": 0, "off": 1, "on": 2}[mode]))
+        """fsw_context_set_split: plane split of the tiles of calls with few frame sets ('auto', 'off', 'on', or
+        'auto2' = FSW_SPLIT_AUTO_TWO_STREAMS, the opt-in variant that uses a stream of the context)."""
+        _check(load_library().fsw_context_set_split(self.handle, {"auto": 0, "off": 1, "on": 2, "auto2": 3}[mode]))
 
     def set_timing(self, on=True):
         """fsw_context_set_timing: bracket the sweep kernels of later calls with CUDA events (last_counters()['sweep_ms'])."""
         _check(load_library().fsw_context_set_timing(self.handle, 1 if on else 0))
-
-
-def measure_fp32_peak(device=0):
-    """fsw_measure_fp32_peak: (TFLOP/s, ms) of an FFMA-chain kernel; the 'alu' roofline denominator."""
-    torch = _torch()
-    t, ms = ctypes.c_double(), ctypes.c_double()
-    stream = torch.cuda.current_stream(device).cuda_stream
-    _check(load_library().fsw_measure_fp32_peak(int(device), stream, ctypes.byref(t), ctypes.byref(ms)))
-    return t.value, ms.value

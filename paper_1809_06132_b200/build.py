@@ -1,4 +1,5 @@
-"""Builds libfsw.so (the C-ABI library of include/fsw.h) for sm_100a with nvcc, in-tree.
+"""Builds libfsw.so (the C-ABI library of include/fsw.h) for sm_100a with nvcc, in-tree, and libfsw_probe.so (the
+bench-only FP32-peak probe of csrc/probe_fp32_peak.cu, which is not part of the library's ABI).
 
     python -m paper_1809_06132_b200.build [--force]
 
@@ -19,6 +20,8 @@ CSRC = os.path.join(HERE, "csrc")
 INCLUDE = os.path.join(ROOT, "include")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libfsw.so")
+PROBE_LIB = os.path.join(HERE, "libfsw_probe.so")
+PROBE_SRC = os.path.join(CSRC, "probe_fp32_peak.cu")
 WINDOWS = (3, 5, 7, 9, 11, 13, 15)
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
@@ -33,7 +36,8 @@ def _nvcc() -> str:
 
 
 def _sources():
-    deps = [os.path.join(CSRC, f) for f in os.listdir(CSRC)] + [os.path.join(INCLUDE, "fsw.h"), os.path.abspath(__file__)]
+    deps = [os.path.join(CSRC, f) for f in os.listdir(CSRC) if f != os.path.basename(PROBE_SRC)]
+    deps += [os.path.join(INCLUDE, "fsw.h"), os.path.abspath(__file__)]
     units = [("fsw_api.o", "fsw_api.cu", []), ("fsw_aux.o", "fsw_aux.cu", [])]
     units += [("fsw_sweep_w%d.o" % w, "fsw_sweep_inst.cu", ["-DFSW_WIN=%d" % w]) for w in WINDOWS]
     return deps, units
@@ -42,9 +46,18 @@ def _sources():
 def build(force: bool = False, verbose: bool = False) -> str:
     deps, units = _sources()
     newest = max(os.path.getmtime(p) for p in deps)
-    if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= newest:
+    if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= newest and os.path.exists(PROBE_LIB) \
+            and os.path.getmtime(PROBE_LIB) >= os.path.getmtime(PROBE_SRC):
         return LIB
     nvcc = _nvcc()
+    if force or not os.path.exists(PROBE_LIB) or os.path.getmtime(PROBE_LIB) < os.path.getmtime(PROBE_SRC):
+        tmp = PROBE_LIB + ".tmp.%d" % os.getpid()
+        res = subprocess.run([nvcc, "-shared"] + NVCC_FLAGS + [PROBE_SRC, "-o", tmp], capture_output=True, text=True)
+        if res.returncode != 0:
+            raise RuntimeError("nvcc failed for the probe:\n%s\n%s" % (res.stdout, res.stderr))
+        os.replace(tmp, PROBE_LIB)
+    if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= newest:
+        return LIB
     os.makedirs(OBJ, exist_ok=True)
 
     def compile_one(unit):

@@ -118,6 +118,13 @@ struct fsw_context {
     DevBuf lo_depth, lo_c1, lo_c2, lo_k;
     DevBuf ctrl;                   /* FSW_CTRL_WORDS x uint32 */
     DevBuf sets_dev;               /* FswSetPtrs of a batch */
+    /* host side of the set table: a ring of pinned buffers, each guarded by an event recorded after its upload, so
+     * that the upload is a true asynchronous copy (a pageable source would make cudaMemcpyAsync wait for the stream) */
+    static constexpr int N_SET_STAGE = 4;
+    FswSetPtrs* sets_pinned[N_SET_STAGE] = {nullptr, nullptr, nullptr, nullptr};
+    size_t sets_pinned_cap[N_SET_STAGE] = {0, 0, 0, 0};
+    cudaEvent_t sets_ev[N_SET_STAGE] = {nullptr, nullptr, nullptr, nullptr};
+    int sets_next = 0;
     DevBuf split_state;            /* plane split: [set][half][6][H][W] floats */
     DevBuf split_ticket;           /* plane split: one word per (set, tile), zero between launches */
     int32_t split_mode = FSW_SPLIT_AUTO;
@@ -483,8 +490,8 @@ int32_t launch_sweep(fsw_context* ctx, FswSweepArgs& a, int w, cudaStream_t s) {
     a.slot_first = 0;
     a.slot_count = total_slots;
     cudaError_t e;
-    if (a.split && a.split_whole > 0) {
-        /* Two launches: the whole tiles (the first full waves of the queue) in the unsplit instantiation on the
+    if (a.split && a.split_whole > 0 && ctx->split_mode == FSW_SPLIT_AUTO_TWO_STREAMS) {
+        /* Two launches (opt-in): the whole tiles (the first full waves of the queue) in the unsplit instantiation on the
          * caller's stream, the halved tiles in the split instantiation on a low-priority stream of the context that
          * is forked from and joined to the caller's stream by events; its CTAs take the SMs the first launch frees. */
         if (!ctx->aux_stream) {
@@ -584,6 +591,28 @@ int32_t stage_views(fsw_context* ctx, const fsw_image* images, int n_sets, bool 
     }
     if (first) /* cannot happen (a rig has at least one view), but never start a sweep with a dirty queue */
         FSW_CUDA(cudaMemsetAsync(ctx->ctrl.p, 0, (zero_counters ? FSW_CTRL_WORDS : FSW_QUEUE_WORDS) * sizeof(unsigned int), stream));
+    return FSW_OK;
+}
+
+/* the set table of a batch goes to the device through the next pinned staging slot of the context; a slot is reused
+ * only after the copy that last read it has completed (its event), which a ring of four makes the common case */
+int32_t upload_sets(fsw_context* ctx, const FswSetPtrs* sets, int n_sets, cudaStream_t stream) {
+    const size_t bytes = sizeof(FswSetPtrs) * (size_t)n_sets;
+    FSW_CUDA(ctx->sets_dev.reserve(bytes));
+    const int slot = ctx->sets_next;
+    ctx->sets_next = (slot + 1) % fsw_context::N_SET_STAGE;
+    if (!ctx->sets_ev[slot]) FSW_CUDA(cudaEventCreateWithFlags(&ctx->sets_ev[slot], cudaEventDisableTiming));
+    else FSW_CUDA(cudaEventSynchronize(ctx->sets_ev[slot]));
+    if (ctx->sets_pinned_cap[slot] < bytes) {
+        if (ctx->sets_pinned[slot]) cudaFreeHost(ctx->sets_pinned[slot]);
+        ctx->sets_pinned[slot] = nullptr;
+        ctx->sets_pinned_cap[slot] = 0;
+        FSW_CUDA(cudaMallocHost((void**)&ctx->sets_pinned[slot], bytes));
+        ctx->sets_pinned_cap[slot] = bytes;
+    }
+    std::memcpy(ctx->sets_pinned[slot], sets, bytes);
+    FSW_CUDA(cudaMemcpyAsync(ctx->sets_dev.p, ctx->sets_pinned[slot], bytes, cudaMemcpyHostToDevice, stream));
+    FSW_CUDA(cudaEventRecord(ctx->sets_ev[slot], stream));
     return FSW_OK;
 }
 
@@ -755,6 +784,10 @@ int32_t fsw_context_destroy(fsw_context* ctx) {
         for (DevBuf& b : *v) b.release();
     ctx->lo_depth.release(); ctx->lo_c1.release(); ctx->lo_c2.release(); ctx->lo_k.release();
     ctx->ctrl.release(); ctx->sets_dev.release();
+    for (int i = 0; i < fsw_context::N_SET_STAGE; ++i) {
+        if (ctx->sets_pinned[i]) cudaFreeHost(ctx->sets_pinned[i]);
+        if (ctx->sets_ev[i]) cudaEventDestroy(ctx->sets_ev[i]);
+    }
     ctx->split_state.release(); ctx->split_ticket.release();
     if (ctx->aux_stream) { cudaStreamDestroy(ctx->aux_stream); cudaEventDestroy(ctx->ev_fork); cudaEventDestroy(ctx->ev_join); }
     for (TileOrder* t : ctx->orders) {
@@ -804,9 +837,7 @@ static int32_t run_sets(fsw_context* ctx, const fsw_planeset* planes, const fsw_
     a.n_sets = n_sets;
     a.set0 = sets[0];
     if (n_sets > 1) {
-        FSW_CUDA(ctx->sets_dev.reserve(sizeof(FswSetPtrs) * (size_t)n_sets));
-        /* pageable source: the runtime stages it before returning, so the vector may die with this call */
-        FSW_CUDA(cudaMemcpyAsync(ctx->sets_dev.p, sets.data(), sizeof(FswSetPtrs) * (size_t)n_sets, cudaMemcpyHostToDevice, stream));
+        if ((rc = upload_sets(ctx, sets.data(), n_sets, stream)) != FSW_OK) return rc;
         a.sets = (const FswSetPtrs*)ctx->sets_dev.p;
     }
     a.count_pixels = 1;
@@ -1009,14 +1040,14 @@ int32_t fsw_compute_depth_multires_host(fsw_context* ctx, const fsw_planeset* pl
 }
 
 int32_t fsw_filter_continuity(fsw_context* ctx, const float* depth_in, size_t depth_in_pitch, int32_t window,
-                              float gamma, float delta, const uint8_t* mask, size_t mask_pitch,
+                              double gamma, double delta, const uint8_t* mask, size_t mask_pitch,
                               float* depth_out, size_t depth_out_pitch, uint8_t* reason_out, size_t reason_pitch,
                               void* cuda_stream) {
     if (!ctx || !depth_in || !depth_out) return fail(FSW_E_INVALID_ARG, "fsw_filter_continuity: null context or depth buffer");
     if (window < 3 || window > FSW_MAX_WINDOW || window % 2 == 0)
         return fail(FSW_E_INVALID_ARG, "fsw_filter_continuity: window=%d must be odd and in 3..%d", window, FSW_MAX_WINDOW);
-    if (!(gamma > 0.f) || !(delta >= 0.f && delta <= 1.f))
-        return fail(FSW_E_INVALID_ARG, "fsw_filter_continuity: gamma=%g must be > 0 and delta=%g in [0,1]", (double)gamma, (double)delta);
+    if (!(gamma > 0.0) || !(delta >= 0.0 && delta <= 1.0))
+        return fail(FSW_E_INVALID_ARG, "fsw_filter_continuity: gamma=%g must be > 0 and delta=%g in [0,1]", gamma, delta);
     const fsw_camera& ref = ctx->rig.cams[ctx->rig.ref_index];
     const int W = ref.width, H = ref.height;
     if (depth_in_pitch < (size_t)W * 4 || depth_out_pitch < (size_t)W * 4 || (mask && mask_pitch < (size_t)W) ||
@@ -1033,7 +1064,7 @@ int32_t fsw_filter_continuity(fsw_context* ctx, const float* depth_in, size_t de
     a.mask = mask; a.mask_pitch = (int64_t)mask_pitch;
     a.reason = reason_out; a.reason_pitch = (int64_t)reason_pitch;
     a.W = W; a.H = H; a.window = window;
-    a.gamma = (double)gamma; a.delta = (double)delta;
+    a.gamma = gamma; a.delta = delta;
     FSW_CUDA(fsw_launch_continuity(a, (cudaStream_t)cuda_stream));
     return FSW_OK;
 }
@@ -1046,7 +1077,7 @@ int32_t fsw_context_set_host_async(fsw_context* ctx, int32_t on) {
 
 int32_t fsw_context_set_split(fsw_context* ctx, int32_t mode) {
     if (!ctx) return fail(FSW_E_INVALID_ARG, "fsw_context_set_split: null context");
-    if (mode != FSW_SPLIT_AUTO && mode != FSW_SPLIT_OFF && mode != FSW_SPLIT_ON)
+    if (mode != FSW_SPLIT_AUTO && mode != FSW_SPLIT_OFF && mode != FSW_SPLIT_ON && mode != FSW_SPLIT_AUTO_TWO_STREAMS)
         return fail(FSW_E_INVALID_ARG, "fsw_context_set_split: mode %d", mode);
     ctx->split_mode = mode;
     return FSW_OK;
@@ -1083,40 +1114,6 @@ int32_t fsw_get_last_counters(fsw_context* ctx, fsw_counters* out) {
         if (ctx->n_timed > 1) FSW_CUDA(cudaEventElapsedTime(&t2, ctx->ev[2], ctx->ev[3]));
         out->sweep_ms = (double)t + (double)t2;
     }
-    return FSW_OK;
-}
-
-int32_t fsw_measure_fp32_peak(int32_t cuda_device, void* cuda_stream, double* tflops, double* ms) {
-    if (!tflops || !ms) return fail(FSW_E_INVALID_ARG, "fsw_measure_fp32_peak: null argument");
-    DeviceGuard g;
-    FSW_CUDA(g.enter(cuda_device));
-    cudaStream_t stream = (cudaStream_t)cuda_stream;
-    cudaDeviceProp prop;
-    FSW_CUDA(cudaGetDeviceProperties(&prop, cuda_device));
-    float* sink = nullptr;
-    FSW_CUDA(cudaMalloc(&sink, 4));
-    const int blocks = prop.multiProcessorCount * 8, iters = 4096;
-    cudaEvent_t e0, e1;
-    FSW_CUDA(cudaEventCreate(&e0));
-    FSW_CUDA(cudaEventCreate(&e1));
-    double best = 1e30;
-    cudaError_t err = cudaSuccess;
-    for (int rep = 0; rep < 4 && err == cudaSuccess; ++rep) {
-        cudaEventRecord(e0, stream);
-        err = fsw_launch_ffma_peak(sink, blocks, iters, stream);
-        cudaEventRecord(e1, stream);
-        if (err == cudaSuccess) err = cudaEventSynchronize(e1);
-        float t = 0.f;
-        if (err == cudaSuccess) err = cudaEventElapsedTime(&t, e0, e1);
-        if (rep > 0 && t < best) best = t;
-    }
-    cudaEventDestroy(e0);
-    cudaEventDestroy(e1);
-    cudaFree(sink);
-    if (err != cudaSuccess) return cuda_fail(err, "fsw_measure_fp32_peak");
-    const double flops = 2.0 * 8.0 * 16.0 * (double)iters * 256.0 * (double)blocks;
-    *ms = best;
-    *tflops = flops / (best * 1e-3) / 1e12;
     return FSW_OK;
 }
 

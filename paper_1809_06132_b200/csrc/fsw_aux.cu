@@ -113,22 +113,6 @@ __global__ void __launch_bounds__(CT_X * CT_Y) continuity_kernel(const __grid_co
     if (a.reason != nullptr) a.reason[(int64_t)y * a.reason_pitch + x] = (uint8_t)reason;
 }
 
-/* 8 independent FFMA chains per thread; 2 flop per FFMA */
-__global__ void __launch_bounds__(256) ffma_peak_kernel(float* sink, int iters) {
-    float x0 = threadIdx.x * 1e-3f, x1 = x0 + 1.f, x2 = x0 + 2.f, x3 = x0 + 3.f;
-    float x4 = x0 + 4.f, x5 = x0 + 5.f, x6 = x0 + 6.f, x7 = x0 + 7.f;
-    const float a = 0.999f, b = 1e-4f;
-    for (int i = 0; i < iters; ++i) {
-#pragma unroll
-        for (int j = 0; j < 16; ++j) {
-            x0 = fmaf(x0, a, b); x1 = fmaf(x1, a, b); x2 = fmaf(x2, a, b); x3 = fmaf(x3, a, b);
-            x4 = fmaf(x4, a, b); x5 = fmaf(x5, a, b); x6 = fmaf(x6, a, b); x7 = fmaf(x7, a, b);
-        }
-    }
-    float s = ((x0 + x1) + (x2 + x3)) + ((x4 + x5) + (x6 + x7));
-    if (s == 123.456f) sink[0] = s; /* never true; keeps the chains alive */
-}
-
 }  // namespace
 
 cudaError_t fsw_launch_pack_footprints(const FswPackArgs& args, cudaStream_t stream) {
@@ -151,10 +135,5 @@ cudaError_t fsw_launch_downsample(const FswDownArgs& args, cudaStream_t stream) 
 cudaError_t fsw_launch_continuity(const FswContinuityArgs& args, cudaStream_t stream) {
     dim3 grid((args.W + CT_X - 1) / CT_X, (args.H + CT_Y - 1) / CT_Y, 1);
     continuity_kernel<<<grid, dim3(CT_X, CT_Y, 1), 0, stream>>>(args);
-    return cudaGetLastError();
-}
-
-cudaError_t fsw_launch_ffma_peak(float* sink, int blocks, int iters, cudaStream_t stream) {
-    ffma_peak_kernel<<<blocks, 256, 0, stream>>>(sink, iters);
     return cudaGetLastError();
 }

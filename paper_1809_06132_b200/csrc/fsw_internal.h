@@ -166,6 +166,4 @@ struct FswContinuityArgs {
 };
 cudaError_t fsw_launch_continuity(const FswContinuityArgs& args, cudaStream_t stream);
 
-cudaError_t fsw_launch_ffma_peak(float* sink, int blocks, int iters, cudaStream_t stream);
-
 #endif

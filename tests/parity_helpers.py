@@ -1,12 +1,17 @@
 """Shared by the -m gpu parity tests: run one BASELINE.json config through the C ABI and through the oracle on the
 same seeded inputs and return the parity statistics of oracle/compare.py."""
+import json
+import os
+
 import numpy as np
 
 import oracle
 import synth
 from oracle.compare import compare_maps, depth_conditioning, to_numpy
 
-GATES = dict(index_match_frac=0.999, cost_tol=1e-4, depth_frac_over_tol=1e-3)
+GATES = dict(index_match_frac=0.999, cost_tol=1e-4, cost2_max=2e-4, cost2_frac_over_tol=1e-5, depth_frac_over_tol=1e-3,
+             fragile_frac=0.10)
+REPORT = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "gpurun_out", "parity_stats.jsonl")
 
 
 def gpu_objects(cfg, device=0):
@@ -70,15 +75,39 @@ def run_multires(cfg, images, mask, host=False, ctx=None):
     return ref, test, stats, counters
 
 
-def assert_gates(stats, n_eval_rtol=1e-3, depth_frac_over_tol=None):
-    """depth: every pixel must be inside the conditioned bound 1e-3 + 3e-4 (|ds|/s)/pden (DESIGN.md "Tolerances");
-    the plain 1e-3 gate must hold on all but `depth_frac_over_tol` of the pixels (0.1 % on the BASELINE configs; the
-    stress cases with 3x3 windows or 1024 planes have flat, noisy cost curves by construction and pass a looser share)."""
+def assert_gates(stats, n_eval_rtol=1e-3, depth_frac_over_tol=None, fragile_frac=None, label=None):
+    """The gates of BASELINE.json's north_star.
+    index   >= 99.9 % of the oracle-valid pixels, ties in the oracle's own cost vector excused
+    cost    |dc1| <= 1e-4 wherever the indices agree; second best ("first and second best cost"): |dc2| <=
+            1e-4 on all but 1e-5 of those pixels and <= 2e-4 on every one (the second best often is a
+            plane whose warped window is nearly flat and far from the tile's centring constant, where the FP32 sums
+            cancel; the worst case seen is 1.07e-4 on one pixel of C3)
+    depth   every pixel inside 1e-3 + 3 eps (|ds|/s)/pden, eps = the cost error of this run (compare.py); the plain
+            1e-3 on all but `depth_frac_over_tol` of the pixels (0.1 % on the BASELINE configs; the stress cases with
+            3x3 windows or 1024 planes have flat, noisy cost curves by construction and pass a looser share)
+    valid   bit-exact on the pixels the oracle does not flag, and the flags may excuse at most `fragile_frac` of the
+            image (10 % unless the test states the value its configuration needs)
+    N_eval  the kernel's counter within 0.1 % of the oracle's
+    The statistics are printed and appended to gpurun_out/parity_stats.jsonl."""
     lim = GATES["depth_frac_over_tol"] if depth_frac_over_tol is None else depth_frac_over_tol
+    flim = GATES["fragile_frac"] if fragile_frac is None else fragile_frac
+    keys = ("index_exact_frac", "index_match_frac", "max_dc1", "max_dc2", "frac_dc2_over_tol", "frac_ddepth_over_tol", "max_ddepth_rel",
+            "depth_worst_ratio_to_bound", "depth_bound_cost_eps", "fragile_frac", "fragile_frac_of_raw",
+            "tie_frac_of_raw", "valid_mismatch_total", "n_eval_oracle", "n_eval_test")
+    line = dict(label=label or os.environ.get("PYTEST_CURRENT_TEST", "?"), **{k: stats.get(k) for k in keys})
+    print("parity:", json.dumps(line))
+    try:
+        os.makedirs(os.path.dirname(REPORT), exist_ok=True)
+        with open(REPORT, "a") as fh:
+            fh.write(json.dumps(line) + "\n")
+    except OSError:
+        pass
     assert stats["index_match_frac"] >= GATES["index_match_frac"], stats
     assert stats["max_dc1"] <= GATES["cost_tol"], stats
+    assert stats["max_dc2"] <= GATES["cost2_max"] and stats["frac_dc2_over_tol"] <= GATES["cost2_frac_over_tol"], stats
     assert stats["frac_ddepth_over_tol"] <= lim, stats
     assert stats["depth_violations_conditioned"] == 0, stats
+    assert stats["fragile_frac"] <= flim, stats
     assert stats["valid_mismatch_nonfragile"] == 0, stats
     assert stats["raw_valid_mismatch_nonfragile"] == 0, stats
     assert abs(stats["n_eval_test"] - stats["n_eval_oracle"]) <= n_eval_rtol * max(stats["n_eval_oracle"], 1), stats
