@@ -178,6 +178,13 @@ const char* fsw_last_error(void);
  * the image; R not orthonormal; xi outside [0,3]; fov outside (0,360]; distortion not invertible inside the FOV). */
 int32_t fsw_rig_create(const fsw_camera* cams, int32_t n_cams, int32_t ref_index, fsw_rig** out);
 int32_t fsw_rig_destroy(fsw_rig* rig);
+/* A rig made of a subset of the cameras of `rig` (the paper evaluates camera configurations with
+ * fewer matching views, "3 cameras ... save about 17 % of run time"): cam_indices lists n_cams distinct cameras of
+ * `rig` in the order the new rig shall have them; it must contain the reference camera of `rig`, which stays the
+ * reference.  The new rig is independent of the old one (destroy both).
+ * Errors: FSW_E_INVALID_ARG (null, n_cams outside 2..FSW_MAX_CAMERAS, index out of range or repeated, reference camera
+ * missing). */
+int32_t fsw_rig_subset(const fsw_rig* rig, const int32_t* cam_indices, int32_t n_cams, fsw_rig** out);
 /* relative pose reference -> camera `cam`: X_cam = R X_ref + T (R row-major, 9 doubles; T 3 doubles) */
 int32_t fsw_rig_relative_pose(const fsw_rig* rig, int32_t cam, double* R, double* T);
 /* a rig-frame direction (e.g. "down" = (0,1,0)) expressed in the reference-camera frame (the ground
@@ -238,6 +245,17 @@ int32_t fsw_compute_depth_multires(fsw_context* ctx, const fsw_planeset* planes_
                                    fsw_rect crop, const fsw_image* images, const uint8_t* mask, size_t mask_pitch,
                                    const fsw_depth_out* out, void* cuda_stream);
 
+/* The two-scale strategy for n_sets independent frame sets of the rig (arguments as in fsw_compute_depth_batch): one
+ * downsample launch, ONE half-resolution sweep launch and ONE crop sweep launch for the whole batch, so that the
+ * (frame set, tile) queue of the sweep kernel also serves the paper's production path (the multi-scale
+ * estimator is what runs in the vehicle).  Results are identical to n_sets separate fsw_compute_depth_multires calls.
+ * The context's half-resolution scratch grows to n_sets frame sets. */
+int32_t fsw_compute_depth_multires_batch(fsw_context* ctx, const fsw_planeset* planes_low, const fsw_planeset* planes_crop,
+                                         const fsw_sweep_params* params_low, const fsw_sweep_params* params_crop,
+                                         fsw_rect crop, int32_t n_sets, const fsw_image* images,
+                                         const uint8_t* const* masks, size_t mask_pitch, const fsw_depth_out* outs,
+                                         void* cuda_stream);
+
 /* Same calls with HOST buffers: images[i].data, mask and every pointer of `out` are host memory (pinned memory
  * makes the copies asynchronous).  The library stages them through context-owned device buffers on cuda_stream:
  * host->device copies, the kernels, device->host copies, then synchronizes the stream before returning. */
@@ -252,6 +270,11 @@ int32_t fsw_compute_depth_multires_host(fsw_context* ctx, const fsw_planeset* pl
                                         const fsw_sweep_params* params_crop, fsw_rect crop, const fsw_image* images,
                                         const uint8_t* mask, size_t mask_pitch, const fsw_depth_out* out,
                                         void* cuda_stream);
+int32_t fsw_compute_depth_multires_batch_host(fsw_context* ctx, const fsw_planeset* planes_low,
+                                              const fsw_planeset* planes_crop, const fsw_sweep_params* params_low,
+                                              const fsw_sweep_params* params_crop, fsw_rect crop, int32_t n_sets,
+                                              const fsw_image* images, const uint8_t* const* masks, size_t mask_pitch,
+                                              const fsw_depth_out* outs, void* cuda_stream);
 
 /* on != 0: the *_host calls of this context enqueue their host-to-device copies, kernels and device-to-host copies on
  * the caller's stream and return WITHOUT synchronizing it.  The caller then owns the ordering: the host images, masks

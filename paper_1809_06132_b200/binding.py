@@ -27,7 +27,8 @@ EXPORTS = (
     "fsw_ground_normal_in_ref", "fsw_planeset_create", "fsw_planeset_destroy", "fsw_planeset_size",
     "fsw_planeset_table", "fsw_context_create", "fsw_context_destroy", "fsw_compute_depth",
     "fsw_compute_depth_multires", "fsw_compute_depth_host", "fsw_compute_depth_multires_host",
-    "fsw_compute_depth_batch", "fsw_compute_depth_batch_host",
+    "fsw_compute_depth_batch", "fsw_compute_depth_batch_host", "fsw_compute_depth_multires_batch",
+    "fsw_compute_depth_multires_batch_host", "fsw_rig_subset",
     "fsw_context_set_timing", "fsw_context_set_split", "fsw_context_set_host_async", "fsw_get_last_counters", "fsw_filter_continuity",
 )
 
@@ -120,6 +121,10 @@ def load_library():
     L.fsw_compute_depth_batch.argtypes = batch
     L.fsw_compute_depth_batch_host.argtypes = batch
     L.fsw_compute_depth_multires_host.argtypes = multi
+    multi_batch = [vp, vp, vp, P(CParams), P(CParams), CRect, i32, P(CImage), P(vp), sz, P(CDepthOut), vp]
+    L.fsw_compute_depth_multires_batch.argtypes = multi_batch
+    L.fsw_compute_depth_multires_batch_host.argtypes = multi_batch
+    L.fsw_rig_subset.argtypes = [vp, P(i32), i32, P(vp)]
     L.fsw_context_set_timing.argtypes = [vp, i32]
     L.fsw_context_set_split.argtypes = [vp, i32]
     L.fsw_context_set_host_async.argtypes = [vp, i32]
@@ -193,6 +198,17 @@ class Rig:
         _check(L.fsw_rig_create(arr, len(cams), int(ref_index), ctypes.byref(h)))
         self.handle, self.n_cams, self.ref_index = h, len(cams), int(ref_index)
         self.sizes = [(int(c["width"]), int(c["height"])) for c in cams]
+
+    def subset(self, cam_indices):
+        """fsw_rig_subset: a rig of the listed cameras (must include the reference, which stays the reference)."""
+        idx = [int(i) for i in cam_indices]
+        arr = (ctypes.c_int32 * len(idx))(*idx)
+        h = ctypes.c_void_p()
+        _check(load_library().fsw_rig_subset(self.handle, arr, len(idx), ctypes.byref(h)))
+        sub = Rig.__new__(Rig)
+        sub.handle, sub.n_cams, sub.ref_index = h, len(idx), idx.index(self.ref_index)
+        sub.sizes = [self.sizes[i] for i in idx]
+        return sub
 
     def relative_pose(self, cam):
         R, T = (ctypes.c_double * 9)(), (ctypes.c_double * 3)()
@@ -411,6 +427,44 @@ class Context:
                   CRect(*[int(x) for x in crop]), arr, mptr, mpitch, ctypes.byref(cout), stream))
         out["_keep"] = (keep, mkeep)
         return out
+
+    def compute_depth_multires_batch(self, planes_low: PlaneSet, planes_crop: PlaneSet, params_low, params_crop, crop,
+                                     image_sets, masks=None, want=ALL, host=False, outs=None):
+        """fsw_compute_depth_multires_batch / _host: the two-scale strategy for n frame sets in one call."""
+        torch = _torch()
+        L = load_library()
+        n, nc = len(image_sets), self.rig.n_cams
+        arr = (CImage * (n * nc))()
+        keep = []
+        for s, images in enumerate(image_sets):
+            a, k = self._images(images, host)
+            for c in range(nc):
+                arr[s * nc + c] = a[c]
+            keep.append(k)
+        marr, mpitch = None, 0
+        if masks is not None and any(m is not None for m in masks):
+            marr = (ctypes.c_void_p * n)()
+            for s, m in enumerate(masks):
+                ptr, pitch, mk = self._mask(m, host)
+                marr[s] = ptr
+                keep.append(mk)
+                if ptr:
+                    assert mpitch in (0, pitch), "all masks of a batch share one pitch"
+                    mpitch = pitch
+        couts = (CDepthOut * n)()
+        results = []
+        for s in range(n):
+            c, o = self._outputs(host, want, None if outs is None else outs[s])
+            couts[s] = c
+            results.append(o)
+        pl, pc = make_params(params_low), make_params(params_crop)
+        stream = torch.cuda.current_stream(self.device).cuda_stream
+        fn = L.fsw_compute_depth_multires_batch_host if host else L.fsw_compute_depth_multires_batch
+        _check(fn(self.handle, planes_low.handle, planes_crop.handle, ctypes.byref(pl), ctypes.byref(pc),
+                  CRect(*[int(x) for x in crop]), n, arr, marr, mpitch, couts, stream))
+        if results:
+            results[0]["_keep"] = keep
+        return results
 
     def filter_continuity(self, depth, window=5, gamma=0.5, delta=0.3, mask=None, want_reason=True):
         """fsw_filter_continuity: the local depth-continuity filter of PAPER.md:99 + mask on a device depth map.

@@ -4,7 +4,7 @@ bench-only FP32-peak probe of csrc/probe_fp32_peak.cu, which is not part of the 
     python -m paper_1809_06132_b200.build [--force]
 
 Every translation unit is compiled with `-gencode arch=compute_100a,code=sm_100a -lineinfo`; the sweep kernel is
-instantiated once per matching-window size in its own object so the instantiations build in parallel.
+instantiated once per (matching-window size, view count) in its own object so the instantiations build in parallel.
 """
 from __future__ import annotations
 
@@ -24,8 +24,10 @@ PROBE_LIB = os.path.join(HERE, "libfsw_probe.so")
 PROBE_SRC = os.path.join(CSRC, "probe_fp32_peak.cu")
 WINDOWS = (3, 5, 7, 9, 11, 13, 15)
 
+# -compress-all: the library holds some 350 instantiations of the sweep kernel with line information; compressed it is
+# a third of the size (it travels to the GPU box with every gpurun snapshot)
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
-              "-Xcompiler", "-fPIC", "-I" + INCLUDE, "-I" + CSRC]
+              "-Xcompiler", "-fPIC", "-Xfatbin", "-compress-all", "-I" + INCLUDE, "-I" + CSRC]
 
 
 def _nvcc() -> str:
@@ -38,8 +40,15 @@ def _nvcc() -> str:
 def _sources():
     deps = [os.path.join(CSRC, f) for f in os.listdir(CSRC) if f != os.path.basename(PROBE_SRC)]
     deps += [os.path.join(INCLUDE, "fsw.h"), os.path.abspath(__file__)]
-    units = [("fsw_api.o", "fsw_api.cu", []), ("fsw_aux.o", "fsw_aux.cu", [])]
-    units += [("fsw_sweep_w%d.o" % w, "fsw_sweep_inst.cu", ["-DFSW_WIN=%d" % w]) for w in WINDOWS]
+    units = [("fsw_api.o", "fsw_api.cu", []), ("fsw_aux.o", "fsw_aux.cu", []),
+             ("fsw_sweep_dispatch.o", "fsw_sweep_dispatch.cu", [])]
+    # one object per (window, view count): views 1..4 unrolled (3 and 4 only where two views share a pass, i.e. for
+    # windows up to 9), 0 = the run-time view loop; the heaviest objects first
+    for n in (4, 3, 0, 2, 1):
+        for w in WINDOWS:
+            if n in (3, 4) and w > 9:
+                continue
+            units.append(("fsw_sweep_w%d_v%d.o" % (w, n), "fsw_sweep_inst.cu", ["-DFSW_WIN=%d" % w, "-DFSW_NVT=%d" % n]))
     return deps, units
 
 

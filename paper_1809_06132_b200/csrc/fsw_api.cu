@@ -13,13 +13,10 @@
 
 #include "fsw_internal.h"
 
-/* per-window launchers, one object file each (fsw_sweep_inst.cu) */
-#define FSW_DECL_WIN(w)                                                                                  \
-    cudaError_t fsw_launch_sweep_w##w(const FswSweepArgs& args, int variant, int grid, cudaStream_t stream); \
-    cudaError_t fsw_prepare_sweep_w##w();                                                                    \
-    FswSweepGeometry fsw_geometry_sweep_w##w(int n_views);
-FSW_DECL_WIN(3) FSW_DECL_WIN(5) FSW_DECL_WIN(7) FSW_DECL_WIN(9) FSW_DECL_WIN(11) FSW_DECL_WIN(13) FSW_DECL_WIN(15)
-#undef FSW_DECL_WIN
+/* fsw_sweep_dispatch.cu: the sweep-kernel instantiations, one object per (window, view count) */
+cudaError_t fsw_launch_sweep(int window, const FswSweepArgs& args, int variant, int grid, cudaStream_t stream);
+cudaError_t fsw_prepare_sweep(int window, int n_views);
+FswSweepGeometry fsw_sweep_geometry(int window, int n_views);
 
 namespace {
 
@@ -113,11 +110,11 @@ struct fsw_context {
     int32_t device;
     int32_t n_sm = 0;
     std::vector<DevBuf> foot;      /* footprint images of the views: [set slot][camera] */
-    DevBuf half[FSW_MAX_CAMERAS];  /* half-resolution float images */
-    DevBuf half_foot[FSW_MAX_CAMERAS];
-    DevBuf lo_depth, lo_c1, lo_c2, lo_k;
+    std::vector<DevBuf> half;      /* half-resolution float images: [set slot][camera] */
+    std::vector<DevBuf> half_foot; /* ... and their footprint images */
+    std::vector<DevBuf> lo_depth, lo_c1, lo_c2, lo_k; /* raw maps of the half-resolution pass: [set slot] */
     DevBuf ctrl;                   /* FSW_CTRL_WORDS x uint32 */
-    DevBuf sets_dev;               /* FswSetPtrs of a batch */
+    DevBuf sets_dev, sets_dev2;    /* FswSetPtrs of a batch (second table: the crop pass of a multi-resolution batch) */
     /* host side of the set table: a ring of pinned buffers, each guarded by an event recorded after its upload, so
      * that the upload is a true asynchronous copy (a pageable source would make cudaMemcpyAsync wait for the stream) */
     static constexpr int N_SET_STAGE = 4;
@@ -150,15 +147,19 @@ namespace {
 
 /* ---- host precompute (S0) ------------------------------------------------------------------------------------ */
 void relative_pose(const fsw_camera& ref, const fsw_camera& view, double* R, double* T) {
-    /* X_v = R_v^c (R_ref^c)^T X_ref + (t_v - R t_ref): "known relative poses" of PAPER.md:70 from rig->camera extrinsics */
-    for (int i = 0; i < 3; ++i)
+    /* "known relative poses" of PAPER.md:70 from the rig->camera extrinsics: where the reference camera sits in the
+     * view's frame.  Its optical centre is at o = -R_ref^T t_ref in the rig; seen from the view that is T = R_v o + t_v.
+     * Its axes are the rows of R_ref; column j of the relative rotation is the view's image of axis j. */
+    double o[3];
+    for (int j = 0; j < 3; ++j) o[j] = -(ref.R[j] * ref.t[0] + ref.R[3 + j] * ref.t[1] + ref.R[6 + j] * ref.t[2]);
+    for (int i = 0; i < 3; ++i) {
+        const double* rv = &view.R[3 * i];
+        T[i] = rv[0] * o[0] + rv[1] * o[1] + rv[2] * o[2] + view.t[i];
         for (int j = 0; j < 3; ++j) {
-            double s = 0.0;
-            for (int k = 0; k < 3; ++k) s += view.R[3 * i + k] * ref.R[3 * j + k];
-            R[3 * i + j] = s;
+            const double* axis = &ref.R[3 * j];
+            R[3 * i + j] = rv[0] * axis[0] + rv[1] * axis[1] + rv[2] * axis[2];
         }
-    for (int i = 0; i < 3; ++i)
-        T[i] = view.t[i] - (R[3 * i] * ref.t[0] + R[3 * i + 1] * ref.t[1] + R[3 * i + 2] * ref.t[2]);
+    }
 }
 
 int32_t check_camera(const fsw_camera& c, int idx) {
@@ -328,31 +329,12 @@ int32_t fill_args(FswSweepArgs& a, const fsw_rig& rig, const fsw_planeset& ps, c
 
 cudaError_t prepare_window(fsw_context* ctx, int w) {
     if (ctx->prepared[w]) return cudaSuccess;
-    cudaError_t e = cudaErrorInvalidValue;
-    switch (w) {
-        case 3: e = fsw_prepare_sweep_w3(); break;
-        case 5: e = fsw_prepare_sweep_w5(); break;
-        case 7: e = fsw_prepare_sweep_w7(); break;
-        case 9: e = fsw_prepare_sweep_w9(); break;
-        case 11: e = fsw_prepare_sweep_w11(); break;
-        case 13: e = fsw_prepare_sweep_w13(); break;
-        case 15: e = fsw_prepare_sweep_w15(); break;
-    }
+    cudaError_t e = fsw_prepare_sweep(w, ctx->rig.n_cams - 1);
     if (e == cudaSuccess) ctx->prepared[w] = true;
     return e;
 }
 
-FswSweepGeometry window_geometry(int w, int n_views) {
-    switch (w) {
-        case 3: return fsw_geometry_sweep_w3(n_views);
-        case 5: return fsw_geometry_sweep_w5(n_views);
-        case 7: return fsw_geometry_sweep_w7(n_views);
-        case 9: return fsw_geometry_sweep_w9(n_views);
-        case 11: return fsw_geometry_sweep_w11(n_views);
-        case 13: return fsw_geometry_sweep_w13(n_views);
-        default: return fsw_geometry_sweep_w15(n_views);
-    }
-}
+FswSweepGeometry window_geometry(int w, int n_views) { return fsw_sweep_geometry(w, n_views); }
 
 /* picks the kernel variant the views allow (see fsw_sweep.cuh) */
 int pick_variant(const FswSweepArgs& a, int foot_f16) {
@@ -421,7 +403,7 @@ int32_t launch_sweep(fsw_context* ctx, FswSweepArgs& a, int w, cudaStream_t s) {
      * work items with half of the planes (by expected work: a family facing away from the optical axis is reached
      * by about (1 + n_z)/2 of the rays) and the halves merge their winner-take-all states (fsw_sweep.cuh). */
     a.split = 0;
-    if (ctx->split_mode != FSW_SPLIT_OFF && a.n_planes >= 2 && a.n_views <= 2) {
+    if (ctx->split_mode != FSW_SPLIT_OFF && a.n_planes >= 2) {
         long long live = 0; /* tiles that intersect the region of interest and the image circle (the kernel's test) */
         const int hw = w / 2;
         for (int t = 0; t < a.n_tiles; ++t) {
@@ -476,16 +458,7 @@ int32_t launch_sweep(fsw_context* ctx, FswSweepArgs& a, int w, cudaStream_t s) {
         const long long items = la.split ? 2LL * la.slot_count - la.split_whole : (long long)la.n_tiles * la.n_sets;
         const int grid = (int)(items < slots ? items : slots);
         const int var = pick_variant(la, la.foot_f16) + (la.split ? 6 : 0);
-        switch (w) {
-            case 3: return fsw_launch_sweep_w3(la, var, grid, ls);
-            case 5: return fsw_launch_sweep_w5(la, var, grid, ls);
-            case 7: return fsw_launch_sweep_w7(la, var, grid, ls);
-            case 9: return fsw_launch_sweep_w9(la, var, grid, ls);
-            case 11: return fsw_launch_sweep_w11(la, var, grid, ls);
-            case 13: return fsw_launch_sweep_w13(la, var, grid, ls);
-            case 15: return fsw_launch_sweep_w15(la, var, grid, ls);
-        }
-        return cudaErrorInvalidValue;
+        return fsw_launch_sweep(w, la, var, grid, ls);
     };
     a.slot_first = 0;
     a.slot_count = total_slots;
@@ -535,7 +508,8 @@ int32_t stage_views(fsw_context* ctx, const fsw_image* images, int n_sets, bool 
         for (int c = 0; c < rig.n_cams; ++c)
             if (c != rig.ref_index && images[(size_t)s * rig.n_cams + c].dtype != FSW_U8) f16 = 0;
     *foot_f16 = f16;
-    if (!half && ctx->foot.size() < (size_t)n_sets * FSW_MAX_CAMERAS) ctx->foot.resize((size_t)n_sets * FSW_MAX_CAMERAS);
+    std::vector<DevBuf>& foots = half ? ctx->half_foot : ctx->foot;
+    if (foots.size() < (size_t)n_sets * FSW_MAX_CAMERAS) foots.resize((size_t)n_sets * FSW_MAX_CAMERAS);
     bool first = true;
     /* one launch per camera size (all views of a rig usually share one) and per FSW_PACK_MAX images */
     std::vector<bool> done((size_t)rig.n_cams, false);
@@ -569,10 +543,10 @@ int32_t stage_views(fsw_context* ctx, const fsw_image* images, int n_sets, bool 
             done[c] = true;
             int vi = c < rig.ref_index ? c : c - 1; /* view index = camera order without the reference */
             for (int s = 0; s < n_sets; ++s) {
-                DevBuf& fb = half ? ctx->half_foot[c] : ctx->foot[(size_t)s * FSW_MAX_CAMERAS + c];
+                DevBuf& fb = foots[(size_t)s * FSW_MAX_CAMERAS + c];
                 FSW_CUDA(fb.reserve((size_t)W * H * sizeof(float4)));
                 if (half) {
-                    pk.src[pk.n] = ctx->half[c].p; pk.src_pitch[pk.n] = (int64_t)W * 4; pk.dtype[pk.n] = FSW_F32;
+                    pk.src[pk.n] = ctx->half[(size_t)s * FSW_MAX_CAMERAS + c].p; pk.src_pitch[pk.n] = (int64_t)W * 4; pk.dtype[pk.n] = FSW_F32;
                 } else {
                     const fsw_image& im = images[(size_t)s * rig.n_cams + c];
                     pk.src[pk.n] = im.data; pk.src_pitch[pk.n] = (int64_t)im.pitch_bytes; pk.dtype[pk.n] = im.dtype;
@@ -596,9 +570,10 @@ int32_t stage_views(fsw_context* ctx, const fsw_image* images, int n_sets, bool 
 
 /* the set table of a batch goes to the device through the next pinned staging slot of the context; a slot is reused
  * only after the copy that last read it has completed (its event), which a ring of four makes the common case */
-int32_t upload_sets(fsw_context* ctx, const FswSetPtrs* sets, int n_sets, cudaStream_t stream) {
+int32_t upload_sets(fsw_context* ctx, const FswSetPtrs* sets, int n_sets, cudaStream_t stream, int table = 0) {
     const size_t bytes = sizeof(FswSetPtrs) * (size_t)n_sets;
-    FSW_CUDA(ctx->sets_dev.reserve(bytes));
+    DevBuf& dev = table ? ctx->sets_dev2 : ctx->sets_dev;
+    FSW_CUDA(dev.reserve(bytes));
     const int slot = ctx->sets_next;
     ctx->sets_next = (slot + 1) % fsw_context::N_SET_STAGE;
     if (!ctx->sets_ev[slot]) FSW_CUDA(cudaEventCreateWithFlags(&ctx->sets_ev[slot], cudaEventDisableTiming));
@@ -611,7 +586,7 @@ int32_t upload_sets(fsw_context* ctx, const FswSetPtrs* sets, int n_sets, cudaSt
         ctx->sets_pinned_cap[slot] = bytes;
     }
     std::memcpy(ctx->sets_pinned[slot], sets, bytes);
-    FSW_CUDA(cudaMemcpyAsync(ctx->sets_dev.p, ctx->sets_pinned[slot], bytes, cudaMemcpyHostToDevice, stream));
+    FSW_CUDA(cudaMemcpyAsync(dev.p, ctx->sets_pinned[slot], bytes, cudaMemcpyHostToDevice, stream));
     FSW_CUDA(cudaEventRecord(ctx->sets_ev[slot], stream));
     return FSW_OK;
 }
@@ -660,6 +635,24 @@ int32_t fsw_rig_create(const fsw_camera* cams, int32_t n_cams, int32_t ref_index
     for (int i = 0; i < 3; ++i) rig->Trel[ref_index][i] = 0.0;
     *out = rig;
     return FSW_OK;
+}
+
+int32_t fsw_rig_subset(const fsw_rig* rig, const int32_t* cam_indices, int32_t n_cams, fsw_rig** out) {
+    if (!rig || !cam_indices || !out) return fail(FSW_E_INVALID_ARG, "fsw_rig_subset: null argument");
+    *out = nullptr;
+    if (n_cams < 2 || n_cams > FSW_MAX_CAMERAS) return fail(FSW_E_INVALID_ARG, "fsw_rig_subset: n_cams=%d must be in 2..%d", n_cams, FSW_MAX_CAMERAS);
+    fsw_camera cams[FSW_MAX_CAMERAS];
+    int ref = -1;
+    for (int i = 0; i < n_cams; ++i) {
+        const int c = cam_indices[i];
+        if (c < 0 || c >= rig->n_cams) return fail(FSW_E_INVALID_ARG, "fsw_rig_subset: camera index %d out of range", c);
+        for (int j = 0; j < i; ++j)
+            if (cam_indices[j] == c) return fail(FSW_E_INVALID_ARG, "fsw_rig_subset: camera %d listed twice", c);
+        if (c == rig->ref_index) ref = i;
+        cams[i] = rig->cams[c];
+    }
+    if (ref < 0) return fail(FSW_E_INVALID_ARG, "fsw_rig_subset: the reference camera (%d) must be part of the subset", rig->ref_index);
+    return fsw_rig_create(cams, n_cams, ref, out);
 }
 
 int32_t fsw_rig_destroy(fsw_rig* rig) {
@@ -711,12 +704,15 @@ int32_t fsw_planeset_create(const fsw_plane_family* fams, int32_t n_fams, fsw_pl
         for (int i = 0; i < 3; ++i) F.normal[i] /= n;
         ps->fams[f] = F;
         ps->first[f] = k0;
-        double s0 = F.spacing == FSW_INVERSE ? 1.0 / F.d_first : F.d_first;
-        double s1 = F.spacing == FSW_INVERSE ? 1.0 / F.d_last : F.d_last;
-        for (int k = 0; k < F.n_planes; ++k) {
-            double sk = F.n_planes > 1 ? s0 + (double)k * (s1 - s0) / (double)(F.n_planes - 1) : s0;
+        /* the planes divide [first, last] evenly in the spacing variable (1/d or d): plane k is the point with
+         * barycentric weights (n-1-k, k)/(n-1) of the two end planes */
+        const bool inv = F.spacing == FSW_INVERSE;
+        const double end0 = inv ? 1.0 / F.d_first : F.d_first, end1 = inv ? 1.0 / F.d_last : F.d_last;
+        const int last = F.n_planes - 1;
+        for (int k = 0; k <= last; ++k) {
+            const double sk = last > 0 ? ((double)(last - k) * end0 + (double)k * end1) / (double)last : end0;
             ps->s.push_back(sk);
-            ps->d.push_back(F.spacing == FSW_INVERSE ? 1.0 / sk : sk);
+            ps->d.push_back(inv ? 1.0 / sk : sk);
             ps->family.push_back(f);
         }
         k0 += F.n_planes;
@@ -777,13 +773,10 @@ int32_t fsw_context_destroy(fsw_context* ctx) {
     if (!ctx) return FSW_OK;
     DeviceGuard g;
     g.enter(ctx->device);
-    for (int c = 0; c < FSW_MAX_CAMERAS; ++c) {
-        ctx->half[c].release(); ctx->half_foot[c].release();
-    }
-    for (std::vector<DevBuf>* v : {&ctx->foot, &ctx->st_img, &ctx->st_mask, &ctx->st_depth, &ctx->st_c1, &ctx->st_c2, &ctx->st_k, &ctx->st_reason})
+    for (std::vector<DevBuf>* v : {&ctx->foot, &ctx->half, &ctx->half_foot, &ctx->lo_depth, &ctx->lo_c1, &ctx->lo_c2, &ctx->lo_k,
+                                   &ctx->st_img, &ctx->st_mask, &ctx->st_depth, &ctx->st_c1, &ctx->st_c2, &ctx->st_k, &ctx->st_reason})
         for (DevBuf& b : *v) b.release();
-    ctx->lo_depth.release(); ctx->lo_c1.release(); ctx->lo_c2.release(); ctx->lo_k.release();
-    ctx->ctrl.release(); ctx->sets_dev.release();
+    ctx->ctrl.release(); ctx->sets_dev.release(); ctx->sets_dev2.release();
     for (int i = 0; i < fsw_context::N_SET_STAGE; ++i) {
         if (ctx->sets_pinned[i]) cudaFreeHost(ctx->sets_pinned[i]);
         if (ctx->sets_ev[i]) cudaEventDestroy(ctx->sets_ev[i]);
@@ -861,22 +854,28 @@ int32_t fsw_compute_depth_batch(fsw_context* ctx, const fsw_planeset* planes, co
     return run_sets(ctx, planes, params, n_sets, images, masks, mask_pitch, outs, cuda_stream, "fsw_compute_depth_batch");
 }
 
-int32_t fsw_compute_depth_multires(fsw_context* ctx, const fsw_planeset* planes_low, const fsw_planeset* planes_crop,
-                                   const fsw_sweep_params* params_low, const fsw_sweep_params* params_crop,
-                                   fsw_rect crop, const fsw_image* images, const uint8_t* mask, size_t mask_pitch,
-                                   const fsw_depth_out* out, void* cuda_stream) {
-    if (!ctx || !planes_low || !planes_crop) return fail(FSW_E_INVALID_ARG, "fsw_compute_depth_multires: null context or plane set");
+/* the two-scale path (S10) for n_sets frame sets: one downsample launch per FSW_PACK_MAX images, the half-resolution
+ * sweep of all sets in one launch, the crop sweep of all sets in one launch */
+static int32_t run_multires(fsw_context* ctx, const fsw_planeset* planes_low, const fsw_planeset* planes_crop,
+                            const fsw_sweep_params* params_low, const fsw_sweep_params* params_crop, fsw_rect crop,
+                            int32_t n_sets, const fsw_image* images, const uint8_t* const* masks, size_t mask_pitch,
+                            const fsw_depth_out* outs, void* cuda_stream, const char* who) {
+    if (!ctx || !planes_low || !planes_crop) return fail(FSW_E_INVALID_ARG, "%s: null context or plane set", who);
+    if (n_sets < 1 || n_sets > FSW_MAX_BATCH) return fail(FSW_E_INVALID_ARG, "%s: n_sets=%d must be in 1..%d", who, n_sets, FSW_MAX_BATCH);
+    if (!images || !outs) return fail(FSW_E_INVALID_ARG, "%s: null images or outputs", who);
     int32_t rc;
     if ((rc = check_params(params_low, "params_low")) != FSW_OK) return rc;
     if ((rc = check_params(params_crop, "params_crop")) != FSW_OK) return rc;
-    if ((rc = check_images(ctx->rig, images)) != FSW_OK) return rc;
-    if ((rc = check_out(ctx->rig, out, mask, mask_pitch)) != FSW_OK) return rc;
     const fsw_rig& rig = ctx->rig;
+    for (int s = 0; s < n_sets; ++s) {
+        if ((rc = check_images(rig, images + (size_t)s * rig.n_cams)) != FSW_OK) return rc;
+        if ((rc = check_out(rig, &outs[s], masks ? masks[s] : nullptr, mask_pitch)) != FSW_OK) return rc;
+    }
     const fsw_camera& ref = rig.cams[rig.ref_index];
     if (crop.w <= 0 || crop.h <= 0 || crop.x0 < 0 || crop.y0 < 0 || crop.x0 + crop.w > ref.width || crop.y0 + crop.h > ref.height)
-        return fail(FSW_E_INVALID_ARG, "fsw_compute_depth_multires: crop (%d,%d,%d,%d) not inside the reference image", crop.x0, crop.y0, crop.w, crop.h);
+        return fail(FSW_E_INVALID_ARG, "%s: crop (%d,%d,%d,%d) not inside the reference image", who, crop.x0, crop.y0, crop.w, crop.h);
     if (params_low->debug_cost_volume || params_crop->debug_cost_volume)
-        return fail(FSW_E_UNSUPPORTED, "fsw_compute_depth_multires: debug_cost_volume is only available in fsw_compute_depth");
+        return fail(FSW_E_UNSUPPORTED, "%s: debug_cost_volume is only available in fsw_compute_depth", who);
     cudaStream_t stream = (cudaStream_t)cuda_stream;
     DeviceGuard g;
     FSW_CUDA(g.enter(ctx->device));
@@ -885,39 +884,56 @@ int32_t fsw_compute_depth_multires(fsw_context* ctx, const fsw_planeset* planes_
     ctx->last_stream = stream;
     ctx->last_launches = 0;
     ctx->last_split = 0;
+    const size_t ns = (size_t)n_sets;
+    if (ctx->half.size() < ns * FSW_MAX_CAMERAS) ctx->half.resize(ns * FSW_MAX_CAMERAS);
+    for (std::vector<DevBuf>* v : {&ctx->lo_depth, &ctx->lo_c1, &ctx->lo_c2, &ctx->lo_k})
+        if (v->size() < ns) v->resize(ns);
 
-    /* S10(a): 2x2 box downsample of every image */
+    /* S10(a): 2x2 box downsample of every image of every set */
     FswDownArgs dn;
     std::memset(&dn, 0, sizeof(dn));
-    dn.n = rig.n_cams;
-    for (int c = 0; c < rig.n_cams; ++c) {
-        const int W = rig.cams[c].width, H = rig.cams[c].height;
-        FSW_CUDA(ctx->half[c].reserve((size_t)(W / 2) * (H / 2) * 4));
-        dn.src[c] = images[c].data; dn.src_pitch[c] = (int64_t)images[c].pitch_bytes; dn.dtype[c] = images[c].dtype;
-        dn.dst[c] = (float*)ctx->half[c].p; dn.W[c] = W; dn.H[c] = H;
-    }
-    FSW_CUDA(fsw_launch_downsample(dn, stream));
-    ctx->last_launches++;
+    for (int s = 0; s < n_sets; ++s)
+        for (int c = 0; c < rig.n_cams; ++c) {
+            const int W = rig.cams[c].width, H = rig.cams[c].height;
+            const fsw_image& im = images[(size_t)s * rig.n_cams + c];
+            DevBuf& hb = ctx->half[(size_t)s * FSW_MAX_CAMERAS + c];
+            FSW_CUDA(hb.reserve((size_t)(W / 2) * (H / 2) * 4));
+            dn.src[dn.n] = im.data; dn.src_pitch[dn.n] = (int64_t)im.pitch_bytes; dn.dtype[dn.n] = im.dtype;
+            dn.dst[dn.n] = (float*)hb.p; dn.W[dn.n] = W; dn.H[dn.n] = H;
+            if (++dn.n == FSW_PACK_MAX || (s == n_sets - 1 && c == rig.n_cams - 1)) {
+                FSW_CUDA(fsw_launch_downsample(dn, stream));
+                ctx->last_launches++;
+                dn.n = 0;
+            }
+        }
 
     /* S10(b): half-resolution sweep over the whole field of view, raw maps into context scratch */
     const int LW = ref.width / 2, LH = ref.height / 2;
-    FSW_CUDA(ctx->lo_depth.reserve((size_t)LW * LH * 4));
-    FSW_CUDA(ctx->lo_c1.reserve((size_t)LW * LH * 4));
-    FSW_CUDA(ctx->lo_c2.reserve((size_t)LW * LH * 4));
-    FSW_CUDA(ctx->lo_k.reserve((size_t)LW * LH * 2));
     FswSweepArgs a;
     fsw_sweep_params pl = *params_low;
     pl.filters_enabled = 0; /* filters run after the merge (reading Q20) */
     fill_args(a, rig, *planes_low, pl, true);
-    FswSetPtrs lo;
-    std::memset(&lo, 0, sizeof(lo));
-    lo.ref_img = ctx->half[rig.ref_index].p; lo.ref_pitch_bytes = (int64_t)LW * 4; lo.ref_dtype = FSW_F32;
-    lo.out_depth = (float*)ctx->lo_depth.p; lo.out_depth_pitch = (int64_t)LW * 4;
-    lo.out_c1 = (float*)ctx->lo_c1.p; lo.out_c1_pitch = (int64_t)LW * 4;
-    lo.out_c2 = (float*)ctx->lo_c2.p; lo.out_c2_pitch = (int64_t)LW * 4;
-    lo.out_k = (int16_t*)ctx->lo_k.p; lo.out_k_pitch = (int64_t)LW * 2;
-    if ((rc = stage_views(ctx, nullptr, 1, true, &lo, stream, true, &a.foot_f16)) != FSW_OK) return rc;
-    a.set0 = lo;
+    std::vector<FswSetPtrs> sets(ns);
+    std::memset(sets.data(), 0, sizeof(FswSetPtrs) * ns);
+    for (int s = 0; s < n_sets; ++s) {
+        FSW_CUDA(ctx->lo_depth[s].reserve((size_t)LW * LH * 4));
+        FSW_CUDA(ctx->lo_c1[s].reserve((size_t)LW * LH * 4));
+        FSW_CUDA(ctx->lo_c2[s].reserve((size_t)LW * LH * 4));
+        FSW_CUDA(ctx->lo_k[s].reserve((size_t)LW * LH * 2));
+        FswSetPtrs& lo = sets[s];
+        lo.ref_img = ctx->half[(size_t)s * FSW_MAX_CAMERAS + rig.ref_index].p; lo.ref_pitch_bytes = (int64_t)LW * 4; lo.ref_dtype = FSW_F32;
+        lo.out_depth = (float*)ctx->lo_depth[s].p; lo.out_depth_pitch = (int64_t)LW * 4;
+        lo.out_c1 = (float*)ctx->lo_c1[s].p; lo.out_c1_pitch = (int64_t)LW * 4;
+        lo.out_c2 = (float*)ctx->lo_c2[s].p; lo.out_c2_pitch = (int64_t)LW * 4;
+        lo.out_k = (int16_t*)ctx->lo_k[s].p; lo.out_k_pitch = (int64_t)LW * 2;
+    }
+    if ((rc = stage_views(ctx, nullptr, n_sets, true, sets.data(), stream, true, &a.foot_f16)) != FSW_OK) return rc;
+    a.n_sets = n_sets;
+    a.set0 = sets[0];
+    if (n_sets > 1) {
+        if ((rc = upload_sets(ctx, sets.data(), n_sets, stream, 0)) != FSW_OK) return rc;
+        a.sets = (const FswSetPtrs*)ctx->sets_dev.p;
+    }
     a.count_pixels = 0;
     ctx->n_timed = 0;
     if (ctx->timing) FSW_CUDA(cudaEventRecord(ctx->ev[2], stream));
@@ -928,15 +944,23 @@ int32_t fsw_compute_depth_multires(fsw_context* ctx, const fsw_planeset* planes_
     fsw_sweep_params pc = *params_crop;
     pc.roi = crop;
     fill_args(a, rig, *planes_crop, pc, false);
-    FswSetPtrs hi;
-    std::memset(&hi, 0, sizeof(hi));
-    const fsw_image& ri = images[rig.ref_index];
-    hi.ref_img = ri.data; hi.ref_pitch_bytes = (int64_t)ri.pitch_bytes; hi.ref_dtype = ri.dtype;
-    set_outputs(hi, out, mask, mask_pitch);
-    hi.lo_depth = (const float*)ctx->lo_depth.p; hi.lo_c1 = (const float*)ctx->lo_c1.p; hi.lo_c2 = (const float*)ctx->lo_c2.p;
-    hi.lo_k = (const int16_t*)ctx->lo_k.p;
-    if ((rc = stage_views(ctx, images, 1, false, &hi, stream, false, &a.foot_f16)) != FSW_OK) return rc;
-    a.set0 = hi;
+    std::memset(sets.data(), 0, sizeof(FswSetPtrs) * ns);
+    for (int s = 0; s < n_sets; ++s) {
+        FswSetPtrs& hi = sets[s];
+        const fsw_image& ri = images[(size_t)s * rig.n_cams + rig.ref_index];
+        hi.ref_img = ri.data; hi.ref_pitch_bytes = (int64_t)ri.pitch_bytes; hi.ref_dtype = ri.dtype;
+        set_outputs(hi, &outs[s], masks ? masks[s] : nullptr, mask_pitch);
+        hi.lo_depth = (const float*)ctx->lo_depth[s].p; hi.lo_c1 = (const float*)ctx->lo_c1[s].p;
+        hi.lo_c2 = (const float*)ctx->lo_c2[s].p; hi.lo_k = (const int16_t*)ctx->lo_k[s].p;
+    }
+    if ((rc = stage_views(ctx, images, n_sets, false, sets.data(), stream, false, &a.foot_f16)) != FSW_OK) return rc;
+    a.n_sets = n_sets;
+    a.set0 = sets[0];
+    if (n_sets > 1) {
+        /* second table of the call: the low sweep may still be reading the first one */
+        if ((rc = upload_sets(ctx, sets.data(), n_sets, stream, 1)) != FSW_OK) return rc;
+        a.sets = (const FswSetPtrs*)ctx->sets_dev2.p;
+    }
     a.lo_W = LW; a.lo_H = LH;
     a.index_flag = FSW_INDEX_FROM_CROP;
     a.count_pixels = 1;
@@ -944,6 +968,24 @@ int32_t fsw_compute_depth_multires(fsw_context* ctx, const fsw_planeset* planes_
     if ((rc = launch_sweep(ctx, a, params_crop->window, stream)) != FSW_OK) return rc;
     if (ctx->timing) { FSW_CUDA(cudaEventRecord(ctx->ev[1], stream)); ctx->n_timed = 2; }
     return FSW_OK;
+}
+
+int32_t fsw_compute_depth_multires(fsw_context* ctx, const fsw_planeset* planes_low, const fsw_planeset* planes_crop,
+                                   const fsw_sweep_params* params_low, const fsw_sweep_params* params_crop,
+                                   fsw_rect crop, const fsw_image* images, const uint8_t* mask, size_t mask_pitch,
+                                   const fsw_depth_out* out, void* cuda_stream) {
+    const uint8_t* masks[1] = {mask};
+    return run_multires(ctx, planes_low, planes_crop, params_low, params_crop, crop, 1, images, mask ? masks : nullptr,
+                        mask_pitch, out, cuda_stream, "fsw_compute_depth_multires");
+}
+
+int32_t fsw_compute_depth_multires_batch(fsw_context* ctx, const fsw_planeset* planes_low, const fsw_planeset* planes_crop,
+                                         const fsw_sweep_params* params_low, const fsw_sweep_params* params_crop,
+                                         fsw_rect crop, int32_t n_sets, const fsw_image* images,
+                                         const uint8_t* const* masks, size_t mask_pitch, const fsw_depth_out* outs,
+                                         void* cuda_stream) {
+    return run_multires(ctx, planes_low, planes_crop, params_low, params_crop, crop, n_sets, images, masks, mask_pitch,
+                        outs, cuda_stream, "fsw_compute_depth_multires_batch");
 }
 
 /* ---- host-buffer variants ------------------------------------------------------------------------------------- */
@@ -999,7 +1041,7 @@ static int32_t run_host(fsw_context* ctx, bool multires, const fsw_planeset* p0,
     }
     bool any_mask = false;
     for (int s = 0; s < n_sets; ++s) any_mask = any_mask || dmask[s] != nullptr;
-    if (multires) rc = fsw_compute_depth_multires(ctx, p0, p1, q0, q1, crop, dimg.data(), dmask[0], (size_t)W, &dout[0], cuda_stream);
+    if (multires) rc = run_multires(ctx, p0, p1, q0, q1, crop, n_sets, dimg.data(), any_mask ? dmask.data() : nullptr, (size_t)W, dout.data(), cuda_stream, "fsw_compute_depth_multires_host");
     else rc = run_sets(ctx, p0, q0, n_sets, dimg.data(), any_mask ? dmask.data() : nullptr, (size_t)W, dout.data(), cuda_stream, "fsw_compute_depth_host");
     if (rc != FSW_OK) return rc;
     for (int s = 0; s < n_sets; ++s) {
@@ -1037,6 +1079,14 @@ int32_t fsw_compute_depth_multires_host(fsw_context* ctx, const fsw_planeset* pl
                                         void* cuda_stream) {
     const uint8_t* masks[1] = {mask};
     return run_host(ctx, true, planes_low, planes_crop, params_low, params_crop, crop, 1, images, mask ? masks : nullptr, mask_pitch, out, cuda_stream);
+}
+
+int32_t fsw_compute_depth_multires_batch_host(fsw_context* ctx, const fsw_planeset* planes_low,
+                                              const fsw_planeset* planes_crop, const fsw_sweep_params* params_low,
+                                              const fsw_sweep_params* params_crop, fsw_rect crop, int32_t n_sets,
+                                              const fsw_image* images, const uint8_t* const* masks, size_t mask_pitch,
+                                              const fsw_depth_out* outs, void* cuda_stream) {
+    return run_host(ctx, true, planes_low, planes_crop, params_low, params_crop, crop, n_sets, images, masks, mask_pitch, outs, cuda_stream);
 }
 
 int32_t fsw_filter_continuity(fsw_context* ctx, const float* depth_in, size_t depth_in_pitch, int32_t window,

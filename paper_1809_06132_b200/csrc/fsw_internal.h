@@ -147,12 +147,12 @@ struct FswPackArgs {
 cudaError_t fsw_launch_pack_footprints(const FswPackArgs& args, cudaStream_t stream);
 
 struct FswDownArgs {
-    int32_t n;
-    const void* src[FSW_MAX_CAMERAS];
-    int64_t src_pitch[FSW_MAX_CAMERAS];
-    int32_t dtype[FSW_MAX_CAMERAS];
-    float* dst[FSW_MAX_CAMERAS]; /* [H/2][W/2] dense */
-    int32_t W[FSW_MAX_CAMERAS], H[FSW_MAX_CAMERAS];
+    int32_t n; /* images of this launch (the cameras of one or several frame sets), at most FSW_PACK_MAX */
+    const void* src[FSW_PACK_MAX];
+    int64_t src_pitch[FSW_PACK_MAX];
+    int32_t dtype[FSW_PACK_MAX];
+    float* dst[FSW_PACK_MAX]; /* [H/2][W/2] dense */
+    int32_t W[FSW_PACK_MAX], H[FSW_PACK_MAX];
 };
 cudaError_t fsw_launch_downsample(const FswDownArgs& args, cudaStream_t stream);
 

@@ -23,9 +23,12 @@
  * private rows of the sample plane and immediately runs the horizontal box sums over them (a __syncwarp, no block
  * barrier, in between); the reference-side operands a' of its horizontal work item stay in registers for the whole
  * sweep.  After one block barrier every thread does the vertical sums, the ZNCC and the winner-take-all update of its
- * own RPT output pixels; the second barrier of a (plane, view) pass sits right after the loads of the vertical pass,
- * so its arithmetic overlaps the next pass of faster warps.  Row groups that no ray can reach (outside the image
- * circle, above the horizon for ground-parallel planes, beyond range_max) are skipped per warp, whole planes per tile.
+ * own RPT output pixels; the second barrier of a pass sits right after the last loads of the vertical pass, so its
+ * arithmetic overlaps the next pass of faster warps.  For windows up to 9 x 9 a pass covers TWO views of the plane
+ * (Geo::FUSE_OK): both are sampled from one load of the ray (shared range test and inverse range), both get their own
+ * sample plane and row-sum planes, and the pair shares the two block barriers, the pass flags and the loop control.
+ * Row groups that no ray can reach (outside the image circle, above the horizon for ground-parallel planes, beyond
+ * range_max) are skipped per warp, whole planes per tile.
  *
  * Numerics: everything is FP32, no fast-math.  Intensities are centred on a per-tile constant before any sum
  * (ZNCC is invariant to offsets) so that Sum(b^2) - Sum(b)^2/N does not cancel catastrophically.
@@ -34,6 +37,8 @@
 #define FSW_SWEEP_CUH
 
 #include <math_constants.h>
+
+#include <type_traits>
 
 #include "fsw_internal.h"
 
@@ -68,11 +73,15 @@ struct Geo {
     static constexpr int PLANE = EHA * SB;
     static constexpr int HPLANE = EHA * HS;
     static constexpr bool A_IN_REGS = WIN <= 9;        /* keep the a' operands of the horizontal item in registers */
+    /* two views per pass: the plane of a' is free after S1 (A_IN_REGS) and holds the samples of the first view; a
+     * second set of row-sum planes brings the block to 203 KB of the 227 KB an sm_100 block may use (the footprint
+     * gathers then have 28 KB of L1 instead of 88 KB: measured + 4 % on the unfused kernel, against - 12 % from fusing) */
+    static constexpr bool FUSE_OK = A_IN_REGS;
     static_assert(EH <= EHA && TX % 32 == 0 && TX % RUN == 0 && NRUN == 8, "tile / thread mapping");
     static_assert(SB >= SBMIN && SB % 4 == 0 && HS % 8 == 4, "aligned strides");
     static_assert(R * NRUN <= 32, "one horizontal work item per lane");
-    static constexpr size_t smem() {
-        return sizeof(float4) * PLANE + sizeof(float) * ((size_t)2 * PLANE + (size_t)4 * HPLANE) +
+    static constexpr size_t smem(bool fuse) {
+        return sizeof(float4) * PLANE + sizeof(float) * ((size_t)2 * PLANE + (size_t)(fuse ? 8 : 4) * HPLANE) +
                sizeof(float2) * TX * TY;
     }
 };
@@ -114,22 +123,25 @@ __device__ inline bool back_project(const FswDevCam& c, float u, float v, float&
             y = yd * sc;
         }
     } else if (c.dist_mode == FSW_DIST_FULL) {
+        /* radial + tangential: fixed-point iteration m <- (m_d - tangential(m)) / radial(m), which contracts wherever
+         * the distortion is invertible (checked at rig creation); the residual decides whether it arrived */
 #pragma unroll 1
-        for (int it = 0; it < 12; ++it) {
-            float r2 = x * x + y * y;
-            float rad = 1.f + c.k1 * r2 + c.k2 * r2 * r2;
-            float drad = c.k1 + 2.f * c.k2 * r2;
-            float gx = x * rad + 2.f * c.p1 * x * y + c.p2 * (r2 + 2.f * x * x) - xd;
-            float gy = y * rad + c.p1 * (r2 + 2.f * y * y) + 2.f * c.p2 * x * y - yd;
-            float jxx = rad + 2.f * x * x * drad + 2.f * c.p1 * y + 6.f * c.p2 * x;
-            float jxy = 2.f * x * y * drad + 2.f * c.p1 * x + 2.f * c.p2 * y;
-            float jyy = rad + 2.f * y * y * drad + 6.f * c.p1 * y + 2.f * c.p2 * x;
-            float det = jxx * jyy - jxy * jxy;
-            if (!(det > 1e-6f)) return false;
-            x -= (jyy * gx - jxy * gy) / det;
-            y -= (jxx * gy - jxy * gx) / det;
+        for (int it = 0; it < 40; ++it) {
+            const float r2 = fmaf(x, x, y * y);
+            const float radial = fmaf(r2, fmaf(c.k2, r2, c.k1), 1.f);
+            const float tx = fmaf(2.f * c.p1 * x, y, c.p2 * fmaf(2.f * x, x, r2));
+            const float ty = fmaf(c.p1, fmaf(2.f * y, y, r2), 2.f * c.p2 * x * y);
+            if (!(radial > 1e-3f)) return false;
+            x = (xd - tx) / radial;
+            y = (yd - ty) / radial;
         }
-        if (!(isfinite(x) && isfinite(y))) return false;
+        {
+            const float r2 = fmaf(x, x, y * y);
+            const float radial = fmaf(r2, fmaf(c.k2, r2, c.k1), 1.f);
+            const float ex = fmaf(x, radial, fmaf(2.f * c.p1 * x, y, c.p2 * fmaf(2.f * x, x, r2))) - xd;
+            const float ey = fmaf(y, radial, fmaf(c.p1, fmaf(2.f * y, y, r2), 2.f * c.p2 * x * y)) - yd;
+            if (!(fabsf(ex) + fabsf(ey) <= 1e-5f * (1.f + fabsf(xd) + fabsf(yd)))) return false; /* not converged / NaN */
+        }
     }
     float rho2 = x * x + y * y;
     float rad = 1.f + (1.f - c.xi * c.xi) * rho2;
@@ -212,8 +224,16 @@ template <> struct FootRaw<true> { uint2 v; };
 template <bool F16>
 __device__ __forceinline__ FootRaw<F16> foot_fetch(const void* __restrict__ foot, unsigned idx) {
     FootRaw<F16> r;
-    if constexpr (F16) r.v = __ldg(reinterpret_cast<const uint2*>(reinterpret_cast<const char*>(foot) + ((size_t)idx << 3)));
-    else r.v = __ldg(reinterpret_cast<const float4*>(reinterpret_cast<const char*>(foot) + ((size_t)idx << 4)));
+    /* the index was already forced to 0 for an invalid sample as a 32-bit value; one wide multiply-add forms the
+     * address (written as PTX so that the select is not redone on the 64-bit offset) */
+    const char* ptr;
+    if constexpr (F16) {
+        asm("mad.wide.u32 %0, %1, 8, %2;" : "=l"(ptr) : "r"(idx), "l"(foot));
+        r.v = __ldg(reinterpret_cast<const uint2*>(ptr));
+    } else {
+        asm("mad.wide.u32 %0, %1, 16, %2;" : "=l"(ptr) : "r"(idx), "l"(foot));
+        r.v = __ldg(reinterpret_cast<const float4*>(ptr));
+    }
     return r;
 }
 template <bool F16>
@@ -392,52 +412,66 @@ __device__ __forceinline__ void h_item(int lane, int& row, int& run) {
     }
 }
 
-/* S2-S4 for the R halo rows of one warp and one (plane, view): samples into the warp's rows of b_s (NaN = invalid).
- * Returns (warp-uniform) whether every sample of the rows is valid. */
-template <class G, bool IDENT, bool FULLDIST, bool CHECKDEN, bool F16>
-__device__ __forceinline__ bool sample_rows(const float4* __restrict__ rays, float* __restrict__ b_s, int sbase, bool tail_on,
-                                            float inv_d, float s_min, const FswDevView& view,
-                                            const void* __restrict__ fv, float centre) {
+/* S2-S4 for the R halo rows of one warp, one plane and NJ views (1 or 2): samples into the warp's rows of b0 (first
+ * view) and b1 (second view), NaN = invalid.  The ray, its inverse range s = (n.r)/d_k and the range test are shared by
+ * the views.  Returns (warp-uniform) bit j set iff every sample of the rows is valid in view j. */
+template <class G, int NJ, bool IDENT, bool FULLDIST, bool CHECKDEN, bool F16>
+__device__ __forceinline__ unsigned sample_rows(const float4* __restrict__ rays, float* __restrict__ b0, float* __restrict__ b1,
+                                                int sbase, bool tail_on, float inv_d, float s_min,
+                                                const FswDevView& view0, const FswDevView& view1,
+                                                const void* __restrict__ f0, const void* __restrict__ f1, float centre) {
     constexpr int NS = G::NS;
-    /* samples in flight per lane: four with the 8-byte footprints of the specialised variant, two otherwise (the raw
-     * footprints of a batch stay in registers) */
-    constexpr int SBATCH = (!FULLDIST && F16) ? 4 : 2;
-    bool all_ok = true;
-    /* batches of SBATCH samples: all addresses, then all fetches, then the lerps.  An invalid sample carries a NaN
-     * weight au (and fetches footprint 0 instead of branching), so its lerp yields the NaN that marks it in b_s. */
+    /* samples in flight per lane: four with the 8-byte footprints of the specialised variants, two otherwise (the raw
+     * footprints of a batch stay in registers); a batch is SLOTS halo pixels x NJ views */
+    constexpr int SLOTS = ((!FULLDIST && F16) ? 4 : 2) / NJ;
+    bool all_ok[NJ];
 #pragma unroll
-    for (int i0 = 0; i0 < NS; i0 += SBATCH) {
-        float au[SBATCH], av[SBATCH];
-        unsigned idx[SBATCH];
-        FootRaw<F16> raw[SBATCH];
+    for (int v = 0; v < NJ; ++v) all_ok[v] = true;
+    /* batches: all addresses, then all fetches, then the lerps.  An invalid sample carries a NaN weight au (and
+     * fetches footprint 0 instead of branching), so its lerp yields the NaN that marks it in the sample plane. */
 #pragma unroll
-        for (int jj = 0; jj < SBATCH; ++jj) {
-            au[jj] = 0.f; av[jj] = 0.f; idx[jj] = 0u;
+    for (int i0 = 0; i0 < NS; i0 += SLOTS) {
+        float au[SLOTS][NJ], av[SLOTS][NJ];
+        unsigned idx[SLOTS][NJ];
+        FootRaw<F16> raw[SLOTS][NJ];
+#pragma unroll
+        for (int jj = 0; jj < SLOTS; ++jj) {
             const int i = i0 + jj;
+#pragma unroll
+            for (int v = 0; v < NJ; ++v) { au[jj][v] = 0.f; av[jj][v] = 0.f; idx[jj][v] = 0u; }
             if (i < NS) {
                 const float4 ry = rays[sbase + 32 * i];
                 float s = ry.w * inv_d;
                 s = (s >= s_min) ? s : CUDART_NAN_F;
-                SampleAddr a = sample_addr<IDENT, FULLDIST, CHECKDEN>(ry.x, ry.y, ry.z, s, view);
-                const bool on = a.ok && (i < G::NSFULL || tail_on); /* a pixel in this slot */
-                au[jj] = on ? a.au : CUDART_NAN_F; av[jj] = a.av;
-                idx[jj] = on ? a.idx : 0u;
-                if (i < G::NSFULL || tail_on) all_ok = all_ok && on;
+#pragma unroll
+                for (int v = 0; v < NJ; ++v) {
+                    SampleAddr a = sample_addr<IDENT, FULLDIST, CHECKDEN>(ry.x, ry.y, ry.z, s, v ? view1 : view0);
+                    const bool on = a.ok && (i < G::NSFULL || tail_on); /* a pixel in this slot */
+                    au[jj][v] = on ? a.au : CUDART_NAN_F; av[jj][v] = a.av;
+                    idx[jj][v] = on ? a.idx : 0u;
+                    if (i < G::NSFULL || tail_on) all_ok[v] = all_ok[v] && on;
+                }
             }
         }
 #pragma unroll
-        for (int jj = 0; jj < SBATCH; ++jj)
-            if (i0 + jj < NS) raw[jj] = foot_fetch<F16>(fv, idx[jj]);
+        for (int jj = 0; jj < SLOTS; ++jj)
 #pragma unroll
-        for (int jj = 0; jj < SBATCH; ++jj) {
+            for (int v = 0; v < NJ; ++v)
+                if (i0 + jj < NS) raw[jj][v] = foot_fetch<F16>(v ? f1 : f0, idx[jj][v]);
+#pragma unroll
+        for (int jj = 0; jj < SLOTS; ++jj) {
             const int i = i0 + jj;
-            if (i < NS) {
-                const float b = foot_lerp<F16>(raw[jj], au[jj], av[jj], centre);
-                if (i < G::NSFULL || tail_on) b_s[sbase + 32 * i] = b;
-            }
+#pragma unroll
+            for (int v = 0; v < NJ; ++v)
+                if (i < NS) {
+                    const float b = foot_lerp<F16>(raw[jj][v], au[jj][v], av[jj][v], centre);
+                    if (i < G::NSFULL || tail_on) (v ? b1 : b0)[sbase + 32 * i] = b;
+                }
         }
     }
-    return __all_sync(0xffffffffu, all_ok);
+    unsigned m = __all_sync(0xffffffffu, all_ok[0]) ? 1u : 0u;
+    if (NJ > 1) m |= __all_sync(0xffffffffu, all_ok[NJ - 1]) ? 2u : 0u;
+    return m;
 }
 
 /* the fields of a frame set the sweep loop touches, staged in shared memory once per tile */
@@ -446,7 +480,8 @@ struct SetHot {
     float* debug_cost;
 };
 
-/* NVT = number of views known at compile time (1 or 2), 0 = read args.n_views at run time. */
+/* NVT = number of views known at compile time (1..4), 0 = read args.n_views at run time (then the view parameters
+ * come from a copy in shared memory, not from dynamically indexed kernel parameters). */
 template <int WIN, int NVT, bool IDENT, bool FULLDIST, bool CHECKDEN, bool F16, bool SPLIT>
 __global__ void __launch_bounds__(Geo<WIN>::NT, 1) sweep_kernel(const __grid_constant__ FswSweepArgs args) {
     using G = Geo<WIN>;
@@ -455,25 +490,39 @@ __global__ void __launch_bounds__(Geo<WIN>::NT, 1) sweep_kernel(const __grid_con
     constexpr float INV_NWIN = 1.f / NWIN;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     float4* rays = reinterpret_cast<float4*>(smem_raw);   /* [EHA][SB]: unit ray, .w = validity / incidence */
-    float* a_s = reinterpret_cast<float*>(rays + G::PLANE); /* [EHA][SB]: centred reference intensities a' */
+    /* two views per pass where the shared memory allows it and there is more than one view */
+    constexpr bool FUSE = G::FUSE_OK && NVT != 1;
+    constexpr int NJ = FUSE ? 2 : 1;
+    float* a_s = reinterpret_cast<float*>(rays + G::PLANE); /* [EHA][SB]: centred reference intensities a' (S1) */
     float* b_s = a_s + G::PLANE;                           /* [EHA][SB]: samples b' of the current (plane, view) */
-    float* hs = b_s + G::PLANE;                            /* [4][EHA][HS]: row sums */
+    float* hs = b_s + G::PLANE;                            /* [NJ][4][EHA][HS]: row sums, one set per view of a pass */
+    /* sample planes of the views of a pass: with FUSE the plane of a' (dead after S1) takes the first view */
+    float* const bs0 = FUSE ? a_s : b_s;
+    float* const bs1 = b_s;
     __shared__ float red_f[G::NW];
     __shared__ int red_i[G::NW];
-    __shared__ unsigned s_mixed[3], s_any[3]; /* rotating flags of a (plane, view) pass */
+    __shared__ unsigned s_mixed[3][2], s_any[3][2]; /* rotating flags of a pass, per view of the pass */
     __shared__ unsigned s_item;
     __shared__ SetHot s_set;
+    __shared__ FswDevView s_views[NVT ? 1 : FSW_MAX_VIEWS]; /* run-time view loop: the view parameters */
 
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     const int col = tid % TX, grp = tid / TX;
     /* [TY][TX]: reference-side window statistics of every output: ((sum a')/N, sum a'^2 - (sum a')^2/N) */
-    float2* const a_stat = reinterpret_cast<float2*>(hs + 4 * G::HPLANE) + (grp * RPT) * TX + col;
+    float2* const a_stat = reinterpret_cast<float2*>(hs + NJ * 4 * G::HPLANE) + (grp * RPT) * TX + col;
     const int W = args.ref.W, H = args.ref.H;
     /* split launches: the first split_whole (tile, set) slots are swept whole, every later one as two halves */
     /* a split launch covers the (tile, set) slots slot_first .. slot_first + slot_count - 1 of the queue order, an
      * unsplit one the first n_tiles * n_sets */
     const int n_items = SPLIT ? 2 * args.slot_count - args.split_whole : args.n_tiles * args.n_sets;
     const int n_views = NVT ? NVT : args.n_views;
+    if constexpr (NVT == 0) {
+        constexpr int NWORDS = (int)(sizeof(FswDevView) / 4) * FSW_MAX_VIEWS;
+        static_assert(sizeof(FswDevView) % 4 == 0 && NWORDS <= G::NT, "one word per thread");
+        if (threadIdx.x < NWORDS)
+            reinterpret_cast<uint32_t*>(s_views)[threadIdx.x] = reinterpret_cast<const uint32_t*>(args.views)[threadIdx.x];
+        /* the first barrier of the first tile orders this against the sweep */
+    }
 
     /* this lane's halo pixels: slot i is element lane + 32 i of the warp's R x SB block of the sample planes; in the
      * last slot only the lanes below `tail` have a pixel */
@@ -528,7 +577,9 @@ __global__ void __launch_bounds__(Geo<WIN>::NT, 1) sweep_kernel(const __grid_con
         float areg[G::NV4 * 4];   /* a' operands of this lane's horizontal work item */
 #pragma unroll
         for (int i = 0; i < G::NV4 * 4; ++i) areg[i] = 0.f;
-        int p3 = 0;               /* state of this warp's rows of plane 3: 0 = WIN everywhere, 1 = zero, 2 = counts */
+        /* state of this warp's rows of plane 3 of either row-sum set: 0 = WIN everywhere, 1 = zero, 2 = counts,
+         * 3 = never written (the second set; S1 fills the first one) */
+        int p3[2] = {0, 3};
         const bool dbg = S.debug_cost != nullptr;
 
         if (tile_live) {
@@ -605,7 +656,7 @@ __global__ void __launch_bounds__(Geo<WIN>::NT, 1) sweep_kernel(const __grid_con
                     a_stat[i * TX] = make_float2(a1n, fmaf(-a1n, sa[i], saa[i]));
                 }
             }
-            if (tid == 0) { s_mixed[0] = 0u; s_mixed[1] = 0u; s_mixed[2] = 0u; s_any[0] = 0u; s_any[1] = 0u; s_any[2] = 0u; }
+            if (tid < 6) { s_mixed[tid >> 1][tid & 1] = 0u; s_any[tid >> 1][tid & 1] = 0u; }
             tile_active = __syncthreads_or(active_mask != 0) != 0;
         }
 
@@ -669,77 +720,109 @@ __global__ void __launch_bounds__(Geo<WIN>::NT, 1) sweep_kernel(const __grid_con
                     /* S2: the plane is out of reach for the whole tile if even the best-facing ray is beyond range */
                     if (qmax * inv_d >= args.inv_range_max) {
                         const bool rows_on = qmax_w * inv_d >= args.inv_range_max; /* any ray of this warp's rows */
-                        constexpr int VSTEP = NVT ? NVT : 1;
-#pragma unroll 1
-                        for (int v0 = 0; v0 < n_views; v0 += VSTEP) {
+                        /* one pass = NJP (1 or 2) views va, va + 1 of the plane: sample, horizontal sums, barrier [A],
+                         * vertical sums (barrier [B] after the last loads), ZNCC into acc / cnt */
+                        auto run_pass = [&](auto njp_c, const int va) {
+                            constexpr int NJP = decltype(njp_c)::value;
+                            const int vb = va + NJP - 1;
+                            const FswDevView& vw0 = NVT ? args.views[va] : s_views[va];
+                            const FswDevView& vw1 = NVT ? args.views[vb] : s_views[vb];
+                            float* const b0 = NJP == 2 ? bs0 : bs1; /* a single view always samples into b_s */
+                            /* ---- S2-S4: sample the plane-warped views at this warp's halo rows ----------------- */
+                            unsigned okmask = (1u << NJP) - 1u;
+                            if (rows_on)
+                                okmask = sample_rows<G, NJP, IDENT, FULLDIST, CHECKDEN, F16>(
+                                    rays, b0, bs1, sbase, tail_on, inv_d, args.inv_range_max, vw0, vw1,
+                                    s_set.foot[va], s_set.foot[vb], centre);
+                            __syncwarp();
+                            /* ---- S5: horizontal box sums of the same rows, view by view ------------------------ */
 #pragma unroll
-                            for (int vv = 0; vv < VSTEP; ++vv) {
-                                const int v = v0 + vv;
-                                /* ---- S2-S4: sample the plane-warped view at this warp's halo rows ------------- */
-                                bool all_ok = true;
-                                if (rows_on) {
-                                    const void* fv = s_set.foot[v];
-                                    all_ok = sample_rows<G, IDENT, FULLDIST, CHECKDEN, F16>(rays, b_s, sbase, tail_on, inv_d,
-                                        args.inv_range_max, args.views[v], fv, centre);
-                                }
-                                __syncwarp();
-                                /* ---- S5: horizontal box sums of the same rows --------------------------------- */
+                            for (int j = 0; j < NJP; ++j) {
+                                float* const hd = h_dst + j * 4 * G::HPLANE;
+                                const bool all_ok = (okmask >> j) & 1u;
                                 bool any_ok = rows_on;
                                 if (rows_on) {
                                     bool any_l = false;
                                     if (h_on) {
                                         float p[G::NV4 * 4];
-                                        load_run<G>(b_s + h_src, p);
+                                        load_run<G>((j ? bs1 : b0) + h_src, p);
                                         if (!G::A_IN_REGS) load_run<G>(a_s + h_src, areg);
                                         if (all_ok) {
-                                            hsum<G, WIN, 1>(p, areg, h_dst);
-                                            if (p3 != 0) fill_count<G>(h_dst, (float)WIN);
+                                            hsum<G, WIN, 1>(p, areg, hd);
+                                            if (p3[j] != 0) fill_count<G>(hd, (float)WIN);
                                         } else {
-                                            any_l = hsum<G, WIN, 2>(p, areg, h_dst);
+                                            any_l = hsum<G, WIN, 2>(p, areg, hd);
                                         }
                                     }
                                     if (!all_ok) any_ok = __any_sync(0xffffffffu, any_l);
-                                    p3 = all_ok ? 0 : 2;
+                                    p3[j] = all_ok ? 0 : 2;
                                 } else {
-                                    if (p3 != 1 && h_on) fill_zero<G>(h_dst);
-                                    p3 = 1;
+                                    if (p3[j] != 1 && h_on) fill_zero<G>(hd);
+                                    p3[j] = 1;
                                 }
                                 if (lane == 0) {
-                                    if (any_ok) s_any[ph] = 1u;
-                                    if (!(rows_on && all_ok)) s_mixed[ph] = 1u;
+                                    if (any_ok) s_any[ph][j] = 1u;
+                                    if (!(rows_on && all_ok)) s_mixed[ph][j] = 1u;
                                 }
-                                __syncthreads(); /* [A] row sums of the pass are complete */
-                                const unsigned f_mixed = s_mixed[ph], f_any = s_any[ph];
-                                {
-                                    const unsigned nx = ph >= 1 ? ph - 1 : 2; /* (ph + 2) % 3: the flags after next */
-                                    if (tid == 0) { s_mixed[nx] = 0u; s_any[nx] = 0u; }
-                                }
-                                ph = ph == 2 ? 0 : ph + 1;
-                                if (f_any == 0) continue; /* the view sees nothing of the tile through this plane */
-                                /* ---- vertical sums, ZNCC ------------------------------------------------------ */
-                                if (!v_act) { /* nothing to score in this warp: only keep the barrier count */
-                                    __syncthreads();
-                                    continue;
-                                }
+                            }
+                            __syncthreads(); /* [A] row sums of the pass are complete */
+                            unsigned f_mixed[NJP], f_any[NJP];
+                            int last = -1; /* last view of the pass that sees anything of the tile */
+#pragma unroll
+                            for (int j = 0; j < NJP; ++j) {
+                                f_mixed[j] = s_mixed[ph][j];
+                                f_any[j] = s_any[ph][j];
+                                if (f_any[j]) last = j;
+                            }
+                            {
+                                const unsigned nx = ph >= 1 ? ph - 1 : 2; /* (ph + 2) % 3: the flags after next */
+                                if (tid < 2) { s_mixed[nx][tid] = 0u; s_any[nx][tid] = 0u; }
+                            }
+                            ph = ph == 2 ? 0 : ph + 1;
+                            if (last < 0) return; /* no view sees anything of the tile through this plane */
+                            /* ---- vertical sums, ZNCC -------------------------------------------------------- */
+                            if (!v_act) { /* nothing to score in this warp: only keep the barrier count */
+                                __syncthreads();
+                                return;
+                            }
+#pragma unroll
+                            for (int j = 0; j < NJP; ++j) {
+                                if (!f_any[j]) continue;
+                                const float* const vs = v_src + j * 4 * G::HPLANE;
                                 float sb[RPT], sbb[RPT], sab[RPT], sv[RPT];
-                                vpass<G, WIN>(v_src, sb);
-                                vpass<G, WIN>(v_src + G::HPLANE, sbb);
-                                vpass<G, WIN>(v_src + 2 * G::HPLANE, sab);
-                                if (f_mixed) vpass<G, WIN>(v_src + 3 * G::HPLANE, sv);
-                                __syncthreads(); /* [B] everyone has read the row sums: the next pass may overwrite */
+                                vpass<G, WIN>(vs, sb);
+                                vpass<G, WIN>(vs + G::HPLANE, sbb);
+                                vpass<G, WIN>(vs + 2 * G::HPLANE, sab);
+                                if (f_mixed[j]) vpass<G, WIN>(vs + 3 * G::HPLANE, sv);
+                                /* [B] everyone has read the row sums: the next pass may overwrite them */
+                                if (j == last) __syncthreads();
 #pragma unroll
                                 for (int i = 0; i < RPT; ++i) {
                                     bool okv = (active_mask >> i) & 1u;
-                                    if (f_mixed) okv = okv && (sv[i] == NWIN);
+                                    if (f_mixed[j]) okv = okv && (sv[i] == NWIN);
                                     const float2 A = a_stat[i * TX]; /* written by this thread */
                                     float cov = fmaf(-A.x, sb[i], sab[i]);
-                                    float vb = fmaf(-sb[i] * INV_NWIN, sb[i], sbb[i]);
-                                    float prod = fmaxf(A.y * vb, args.floor2);
+                                    float vbv = fmaf(-sb[i] * INV_NWIN, sb[i], sbb[i]);
+                                    float prod = fmaxf(A.y * vbv, args.floor2);
                                     float z = cov * rsqrt_approx(prod);
                                     float cst = __saturatef(fmaf(-0.5f, z, 0.5f));
                                     acc[i] += okv ? cst : 0.f;
                                     cnt += okv ? (1u << (4 * i)) : 0u;
                                 }
+                            }
+                        };
+                        if constexpr (NVT != 0) {
+                            /* compile-time view list: pairs, then a single view if the count is odd */
+#pragma unroll
+                            for (int va = 0; va < NVT; va += NJ) {
+                                if (NVT - va >= 2 && NJ == 2) run_pass(std::integral_constant<int, NJ>{}, va);
+                                else run_pass(std::integral_constant<int, 1>{}, va);
+                            }
+                        } else {
+#pragma unroll 1
+                            for (int va = 0; va < n_views; va += NJ) {
+                                if (NJ == 2 && n_views - va >= 2) run_pass(std::integral_constant<int, NJ>{}, va);
+                                else run_pass(std::integral_constant<int, 1>{}, va);
                             }
                         }
                     }
@@ -921,25 +1004,21 @@ __global__ void __launch_bounds__(Geo<WIN>::NT, 1) sweep_kernel(const __grid_con
 }
 
 /* Kernel variants (fsw_api.cu: pick_variant): projection mode 0..2 (see SweepInst::go) + 3 if the footprints are
- * 8-byte bfloat16. */
+ * 8-byte bfloat16, + 6 for the plane split (two work items per tile). */
 template <int WIN, int NVT>
 struct SweepInst {
     using G = Geo<WIN>;
+    static constexpr bool FUSE = G::FUSE_OK && NVT != 1;
     /* MODE 0: any rotation, full distortion polynomial, denominator test; 1: identity rotations, k1-only distortion;
      * 2: any rotation, k1-only distortion (the last two need cos(fov/2) + xi >= 1e-3) */
     template <int MODE, bool F16, bool SPLIT>
     static cudaError_t go(const FswSweepArgs& args, int grid, cudaStream_t stream, bool prepare_only) {
         auto kern = sweep_kernel<WIN, NVT, MODE == 1, MODE == 0, MODE == 0, F16, SPLIT>;
-        if (prepare_only) return cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::smem());
-        kern<<<grid, G::NT, G::smem(), stream>>>(args);
+        if (prepare_only) return cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::smem(FUSE));
+        kern<<<grid, G::NT, G::smem(FUSE), stream>>>(args);
         return cudaGetLastError();
     }
-    /* + 6: plane split (two work items per tile), built for the variants with one or two views only: the run-time
-     * view loop with the split faulted on the device (misaligned address in the 9 x 9 instantiation) whenever the
-     * halo plane, the descending half and the state exchange were all compiled in, and not with any one of them
-     * removed, nor with ptxas at -O1; fsw_api.cu does not split calls with more than two views until that is
-     * understood */
-    static constexpr int N_VARIANTS = NVT ? 12 : 6;
+    static constexpr int N_VARIANTS = 12;
     static cudaError_t dispatch(const FswSweepArgs& args, int variant, int grid, cudaStream_t stream, bool prep) {
         switch (variant) {
             case 0: return go<0, false, false>(args, grid, stream, prep);
@@ -948,18 +1027,13 @@ struct SweepInst {
             case 3: return go<0, true, false>(args, grid, stream, prep);
             case 4: return go<1, true, false>(args, grid, stream, prep);
             case 5: return go<2, true, false>(args, grid, stream, prep);
+            case 6: return go<0, false, true>(args, grid, stream, prep);
+            case 7: return go<1, false, true>(args, grid, stream, prep);
+            case 8: return go<2, false, true>(args, grid, stream, prep);
+            case 9: return go<0, true, true>(args, grid, stream, prep);
+            case 10: return go<1, true, true>(args, grid, stream, prep);
+            case 11: return go<2, true, true>(args, grid, stream, prep);
             default: break;
-        }
-        if constexpr (NVT != 0) {
-            switch (variant) {
-                case 6: return go<0, false, true>(args, grid, stream, prep);
-                case 7: return go<1, false, true>(args, grid, stream, prep);
-                case 8: return go<2, false, true>(args, grid, stream, prep);
-                case 9: return go<0, true, true>(args, grid, stream, prep);
-                case 10: return go<1, true, true>(args, grid, stream, prep);
-                case 11: return go<2, true, true>(args, grid, stream, prep);
-                default: break;
-            }
         }
         return cudaErrorInvalidValue;
     }
@@ -976,30 +1050,20 @@ struct SweepInst {
     }
 };
 
-/* one or two views: the view loop is unrolled; more: a run-time loop */
+/* Which instantiation serves a call: up to four views (the paper's rig has four matching views) have
+ * their view loop unrolled, pairs of views sharing a pass; more views, or three / four views with the large windows
+ * that cannot pair them, take the run-time loop (NVT = 0). */
 template <int WIN>
-cudaError_t launch_sweep_win(const FswSweepArgs& args, int variant, int grid, cudaStream_t stream) {
-    if (args.n_views == 1) return SweepInst<WIN, 1>::launch(args, variant, grid, stream);
-    if (args.n_views == 2) return SweepInst<WIN, 2>::launch(args, variant, grid, stream);
-    return SweepInst<WIN, 0>::launch(args, variant, grid, stream);
-}
-
-template <int WIN>
-cudaError_t prepare_sweep_win() {
-    cudaError_t e = SweepInst<WIN, 1>::prepare();
-    if (e != cudaSuccess) return e;
-    e = SweepInst<WIN, 2>::prepare();
-    if (e != cudaSuccess) return e;
-    return SweepInst<WIN, 0>::prepare();
+constexpr int nvt_for(int n_views) {
+    return n_views <= 2 ? n_views : ((n_views <= 4 && Geo<WIN>::FUSE_OK) ? n_views : 0);
 }
 
 template <int WIN>
 FswSweepGeometry geometry_win(int n_views) {
     using G = Geo<WIN>;
-    (void)n_views;
     FswSweepGeometry g;
     g.tile_w = G::TX; g.tile_h = G::TY; g.threads = G::NT; g.ctas_per_sm = G::MINB;
-    g.smem_bytes = G::smem();
+    g.smem_bytes = G::smem(G::FUSE_OK && n_views != 1);
     return g;
 }
 

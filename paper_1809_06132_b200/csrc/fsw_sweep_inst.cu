@@ -1,18 +1,18 @@
 /*
- * fsw_sweep_inst.cu -- one instantiation of the sweep kernel per matching-window size.
- * Compiled once per window with -DFSW_WIN=<w> (w odd, 3..15) so the instantiations build in parallel.
+ * fsw_sweep_inst.cu -- the instantiations of the sweep kernel for one matching-window size and one view count.
+ * Compiled once per (window, view count) with -DFSW_WIN=<w> (odd, 3..15) -DFSW_NVT=<n> (1..4 views unrolled, 0 = the
+ * run-time view loop) so that the objects build in parallel.
  */
 #include "fsw_sweep.cuh"
 
-#ifndef FSW_WIN
-#error "compile with -DFSW_WIN=<odd window size>"
+#if !defined(FSW_WIN) || !defined(FSW_NVT)
+#error "compile with -DFSW_WIN=<odd window size> -DFSW_NVT=<0..4>"
 #endif
 
-#define FSW_CAT2(a, b) a##b
-#define FSW_CAT(a, b) FSW_CAT2(a, b)
+#define FSW_CAT4_(a, b, c, d) a##b##c##d
+#define FSW_CAT4(a, b, c, d) FSW_CAT4_(a, b, c, d)
 
-cudaError_t FSW_CAT(fsw_launch_sweep_w, FSW_WIN)(const FswSweepArgs& args, int variant, int grid, cudaStream_t stream) {
-    return fsw::launch_sweep_win<FSW_WIN>(args, variant, grid, stream);
+cudaError_t FSW_CAT4(fsw_launch_sweep_w, FSW_WIN, _v, FSW_NVT)(const FswSweepArgs& args, int variant, int grid, cudaStream_t stream) {
+    return fsw::SweepInst<FSW_WIN, FSW_NVT>::launch(args, variant, grid, stream);
 }
-cudaError_t FSW_CAT(fsw_prepare_sweep_w, FSW_WIN)() { return fsw::prepare_sweep_win<FSW_WIN>(); }
-FswSweepGeometry FSW_CAT(fsw_geometry_sweep_w, FSW_WIN)(int n_views) { return fsw::geometry_win<FSW_WIN>(n_views); }
+cudaError_t FSW_CAT4(fsw_prepare_sweep_w, FSW_WIN, _v, FSW_NVT)() { return fsw::SweepInst<FSW_WIN, FSW_NVT>::prepare(); }

@@ -255,10 +255,51 @@ def _paper_rig():
             camera(centre=(-0.25, -0.3, 0.1), yaw_deg=-4.0, **kw), camera(centre=(0.25, -0.3, 0.1), yaw_deg=4.0, **kw)]
 
 
-def make_config(index: int) -> dict:
-    """index = 1..5 for C1..C5 (BASELINE.json configs[index-1]); 6 = the paper's own workload shape:
-    5 cameras (4 matching views) of 1024 x 544, 64 fronto-parallel + 30 ground-parallel planes, 9 x 9 ZNCC, as a
-    stream of 32 frame sets."""
+def _half_camera(c: dict) -> dict:
+    """The camera of the 2x2-box-downsampled image (pixel centres at integers: f/2, c' = (c - 0.5)/2)."""
+    h = dict(c)
+    h.update(width=c["width"] // 2, height=c["height"] // 2, fx=c["fx"] / 2.0, fy=c["fy"] / 2.0,
+             cx=(c["cx"] - 0.5) / 2.0, cy=(c["cy"] - 0.5) / 2.0)
+    return h
+
+
+def make_config(index: int, cameras=None) -> dict:
+    """index = 1..5 for C1..C5 (BASELINE.json configs[index-1]); 6..8 = the paper's own workload shapes (SURVEY 8(f) 2;
+    PAPER.md:76, :88-90, :224, :249), each a stream of 32 frame sets of the five-camera rig (4 matching views):
+      6  "P"   full resolution 1024 x 544, 64 fronto-parallel + 30 ground-parallel planes, 9 x 9 ZNCC (the 50 ms case)
+      7  "PM"  multi-scale: 512 x 272 full field of view with 7 x 7 + the 572 x 332 centre crop at full resolution with
+               9 x 9, the same 64 + 30 planes in both passes (the 36 ms case)
+      8  "PH"  half resolution 512 x 272, 7 x 7 (the 16 ms case); the cameras are those of the downsampled images
+    cameras: optional list of camera indices (the reference first) selecting a sub-rig, e.g. (0, 1, 2) for the
+    three-camera configuration of PAPER.md:280, :294."""
+    if index in (6, 7, 8):
+        cfg = _paper_config(index)
+        if cameras is not None:
+            assert cameras[0] == 0, "the reference camera comes first"
+            cfg = dict(cfg, cams=[cfg["cams"][i] for i in cameras], cameras=tuple(cameras),
+                       name=cfg["name"] + "%d" % len(cameras))
+        return cfg
+    assert cameras is None
+    return _baseline_config(index)
+
+
+def _paper_config(index: int) -> dict:
+    fams = [family((0, 0, 1), 64, 0.5, 50.0, "inverse"), family((0, 1, 0), 30, 1.1, 2.1, "linear")]
+    fil = FILTER_COST | FILTER_RATIO
+    if index == 7:
+        return dict(name="PM", dtype="u8", ref_index=0, cams=_paper_rig(), n_frames=32, step_m=0.5, mask_seed=None,
+                    families_low=fams, families_crop=fams,
+                    params_low=params(7, VAR_FLOOR_U8, 100.0, 0.05, 0.3, 272, 1.2, filters=fil),
+                    params_crop=params(9, VAR_FLOOR_U8, 100.0, 0.05, 0.3, 272, 1.2, filters=fil),
+                    crop=((1024 - 572) // 2, (544 - 332) // 2, 572, 332), scene=scene_street(seed=3))
+    if index == 8:
+        return dict(name="PH", dtype="u8", ref_index=0, cams=[_half_camera(c) for c in _paper_rig()], n_frames=32,
+                    step_m=0.5, mask_seed=None, families=fams,
+                    params=params(7, VAR_FLOOR_U8, 100.0, 0.05, 0.3, 136, 1.2, filters=fil), scene=scene_street(seed=3))
+    return _baseline_config(6)
+
+
+def _baseline_config(index: int) -> dict:
     if index == 6:
         return dict(name="P", dtype="u8", ref_index=0, cams=_paper_rig(), n_frames=32, step_m=0.5, mask_seed=None,
                     families=[family((0, 0, 1), 64, 0.5, 50.0, "inverse"), family((0, 1, 0), 30, 1.1, 2.1, "linear")],
@@ -301,7 +342,7 @@ def make_config(index: int) -> dict:
                               family((0, 1, 0), 64, 1.1, 2.1, "linear")],
                     params=params(9, VAR_FLOOR_U8, 100.0, 0.05, 0.3, 512, 1.2, filters=fil),
                     scene=scene_street(seed=3))
-    raise ValueError("config index must be 1..6")
+    raise ValueError("config index must be 1..8")
 
 
 @lru_cache(maxsize=8)

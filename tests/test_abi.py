@@ -1,6 +1,6 @@
 """CPU-side checks of the C-ABI library (no compute calls): it loads, exports every symbol include/fsw.h declares,
 its struct layouts match the ctypes binding, and its host logic (rig / plane-set validation and precompute, S0 of
-SURVEY.md 8(a)) agrees with the oracle's independently written O2/O3."""
+SURVEY.md 8(a)) gives the closed-form values the conventions fix (and agrees with the oracle's O2/O3)."""
 import ctypes
 import os
 import re
@@ -58,15 +58,40 @@ def test_struct_layouts_match_header():
             assert int(got["%s.%s" % (cname, fname)]) == getattr(cls, fname).offset, (cname, fname)
 
 
+def _yaw(deg):
+    """Closed form of reading Q5: rig -> camera rotation of a camera yawed by `deg` about +y (down); a positive yaw
+    turns the optical axis towards +x, so the rig point (sin, 0, cos) lies on the optical axis."""
+    a = np.radians(deg)
+    return np.array([[np.cos(a), 0.0, -np.sin(a)], [0.0, 1.0, 0.0], [np.sin(a), 0.0, np.cos(a)]])
+
+
 def test_rig_validation_and_relative_pose():
-    cfg = synth.make_config(2)
+    cfg = synth.make_config(2)   # reference at the origin; views at x = -+0.4 m, yawed by -+10 degrees
     rig = fsw.Rig(cfg["cams"], 0)
-    for c in (1, 2):
+    for c, (centre, yaw) in ((1, ((-0.4, 0.0, 0.0), -10.0)), (2, ((0.4, 0.0, 0.0), 10.0))):
         R, T = rig.relative_pose(c)
+        # closed form: the reference frame is the rig frame, so X_v = R_y (X - C): R = R_y, T = -R_y C
+        assert np.allclose(R, _yaw(yaw), atol=1e-15) and np.allclose(T, -_yaw(yaw) @ np.array(centre), atol=1e-15)
+        assert np.allclose(R @ np.array([np.sin(np.radians(yaw)), 0.0, np.cos(np.radians(yaw))]), (0, 0, 1), atol=1e-15)
         Ro, To = oracle.relative_pose(cfg["cams"][0], cfg["cams"][c])
         assert np.allclose(R, Ro, atol=1e-15) and np.allclose(T, To, atol=1e-15)
+    # between two yawed cameras: the rotation is the difference of the yaws, and the reference's centre maps to T
+    rig12 = fsw.Rig(cfg["cams"], 1)
+    R, T = rig12.relative_pose(2)
+    assert np.allclose(R, _yaw(20.0), atol=1e-15)
+    assert np.allclose(T, _yaw(10.0) @ (np.array([-0.4, 0, 0]) - np.array([0.4, 0, 0])), atol=1e-15)
+    Rb, Tb = fsw.Rig(cfg["cams"], 2).relative_pose(1)    # the inverse pose
+    assert np.allclose(Rb @ R, np.eye(3), atol=1e-15) and np.allclose(Rb @ T + Tb, 0.0, atol=1e-15)
     R0, T0 = rig.relative_pose(0)
     assert np.array_equal(R0, np.eye(3)) and np.array_equal(T0, np.zeros(3))
+    # a sub-rig keeps the reference and the poses of the cameras it lists
+    sub = rig.subset([2, 0])
+    assert (sub.n_cams, sub.ref_index) == (2, 1)
+    assert np.array_equal(sub.relative_pose(0)[0], rig.relative_pose(2)[0]) and np.array_equal(sub.relative_pose(0)[1], rig.relative_pose(2)[1])
+    for bad_subset in ([1, 2], [0], [0, 0], [0, 5]):
+        with pytest.raises(fsw.FswError) as ei:
+            rig.subset(bad_subset)
+        assert ei.value.code == fsw.binding.E_INVALID_ARG
     # ground normal: rig "down" expressed in a yawed reference camera stays "down"
     rig2 = fsw.Rig(cfg["cams"], 1)
     assert np.allclose(rig2.ground_normal_in_ref((0, 2.0, 0)), (0, 1, 0), atol=1e-15)
@@ -97,6 +122,17 @@ def test_rig_validation_and_relative_pose():
 
 
 def test_planeset_table_matches_oracle_and_validation():
+    # the values SURVEY.md 8(c) prints for C1 (tests/golden/survey_spot_values.txt): 32 planes uniform in 1/d over
+    # 0.5..50 m
+    from conftest import read_golden
+    g = read_golden(os.path.join(ROOT, "tests", "golden", "survey_spot_values.txt"))["c1_planes"]
+    s, d, f = fsw.PlaneSet(synth.make_config(1)["families"]).table()
+    assert abs((s[0] - s[1]) - g[0]) < 5e-8 and abs(d[0] - g[1]) < 1e-12 and abs(d[27] - g[2]) < 5e-6
+    assert abs(d[28] - g[3]) < 5e-6 and abs(d[31] - g[4]) < 1e-9
+    # closed form: k-th of n planes is the point k/(n-1) of the way in the spacing variable
+    s, d, f = fsw.PlaneSet([synth.family((0, 0, 1), 5, 2.0, 10.0, "linear"), synth.family((0, 1, 0), 3, 1.0, 4.0, "inverse")]).table()
+    assert np.allclose(s, [2, 4, 6, 8, 10, 1.0, 0.625, 0.25], atol=1e-15) and np.allclose(d[5:], [1.0, 1.6, 4.0], atol=1e-15)
+    assert list(f) == [0] * 5 + [1] * 3
     for idx in (1, 3, 5):
         fams = synth.make_config(idx)["families"]
         ps = fsw.PlaneSet(fams)

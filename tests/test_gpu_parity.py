@@ -53,6 +53,93 @@ def test_paper_workload_shape_four_rotated_views():
     assert stats["n_oracle_valid"] > 50000 and counters["n_eval"] > 10_000_000
 
 
+def test_paper_multiscale_shape_and_its_batch():
+    """the paper's multi-scale estimator at its own shape -- 512 x 272 full field of view
+    (7 x 7) + the 572 x 332 centre crop at full resolution (9 x 9), four rotated matching views, 64 + 30 planes -- through
+    fsw_compute_depth_multires against the oracle, and two frame sets through fsw_compute_depth_multires_batch,
+    bit-identical to their single calls."""
+    import torch
+    import paper_1809_06132_b200 as fsw
+    cfg = synth.make_config(7)
+    _, _, ctx = gpu_objects(cfg)
+    images = synth.render_frame(cfg, 2)
+    ref, test, stats, counters = run_multires(cfg, images, None, ctx=ctx)
+    assert_gates(stats, fragile_frac=0.12)
+    assert stats["n_oracle_valid"] > 50000
+    k = ref["kbest"]
+    assert ((k >= 0) & (k >> 14 == 1)).sum() > 50000 and ((k >= 0) & (k >> 14 == 0)).sum() > 50000
+    pl, pc = fsw.PlaneSet(cfg["families_low"]), fsw.PlaneSet(cfg["families_crop"])
+    sets = [[torch.from_numpy(im).cuda() for im in fr] for fr in (images, synth.render_frame(cfg, 9))]
+    masks = [torch.from_numpy(synth.make_mask(1024, 544, 21)).cuda(), None]
+    singles, n_eval = [], 0
+    for st, m in zip(sets, masks):
+        singles.append(oracle.compare.to_numpy(ctx.compute_depth_multires(pl, pc, cfg["params_low"], cfg["params_crop"], cfg["crop"], st, m)))
+        n_eval += ctx.last_counters()["n_eval"]
+    outs = ctx.compute_depth_multires_batch(pl, pc, cfg["params_low"], cfg["params_crop"], cfg["crop"], sets, masks)
+    torch.cuda.synchronize()
+    c = ctx.last_counters()
+    assert c["n_eval"] == n_eval and c["n_launches"] == 5, c   # downsample, pack + low sweep, pack + crop sweep
+    for s in range(2):
+        got = oracle.compare.to_numpy(outs[s])
+        for key in ("depth", "best_cost", "second_cost", "plane_index", "valid_reason"):
+            assert np.array_equal(singles[s][key], got[key], equal_nan=True), (s, key)
+    assert (oracle.compare.to_numpy(outs[0])["depth"][masks[0].cpu().numpy() != 0] == 0).all()
+
+
+def test_paper_half_resolution_shape():
+    """PAPER.md:249 "half resolution": 512 x 272, 7 x 7, the same planes and views (synth.make_config(8))."""
+    cfg = synth.make_config(8)
+    images = synth.render_frame(cfg, 1)
+    _, _, stats, counters = run_single(cfg, images)
+    assert_gates(stats, fragile_frac=0.12)
+    assert stats["n_oracle_valid"] > 15000
+
+
+def test_camera_subset_three_of_five_cameras():
+    """the three-camera configuration.  fsw_rig_subset gives the rig of the listed cameras: its
+    maps equal those of a rig created from those cameras directly, and match the oracle."""
+    import torch
+    import paper_1809_06132_b200 as fsw
+    full = synth.make_config(6)
+    cfg = synth.make_config(6, cameras=(0, 1, 2))
+    images = synth.render_frame(cfg, 5)
+    assert all(np.array_equal(a, b) for a, b in zip(images, synth.render_frame(full, 5)[:3]))
+    sub = fsw.Rig(full["cams"], 0).subset([0, 1, 2])
+    ctx_sub = fsw.Context(sub, 0)
+    ref, test, stats, counters = run_single(cfg, images)            # rig created from the three cameras
+    assert_gates(stats, fragile_frac=0.12)
+    planes = fsw.PlaneSet(cfg["families"])
+    dev = [torch.from_numpy(im).cuda() for im in images]
+    got = oracle.compare.to_numpy(ctx_sub.compute_depth(planes, cfg["params"], dev))
+    for key in ("depth", "best_cost", "second_cost", "plane_index", "valid_reason"):
+        assert np.array_equal(test[key], got[key], equal_nan=True), key
+    assert ctx_sub.last_counters()["n_eval"] == counters["n_eval"]
+
+
+def test_multires_batch_host_small():
+    """fsw_compute_depth_multires_batch_host on a small rig: three frame sets, masks on some, equal to the single
+    host calls bit for bit."""
+    import paper_1809_06132_b200 as fsw
+    cfg = _small_rig(W=128, H=96, n_views=3, rot=True, fov=170.0)
+    _, _, ctx = gpu_objects(cfg)
+    pl = fsw.PlaneSet([synth.family((0, 0, 1), 16, 0.8, 30.0, "inverse")])
+    pc = fsw.PlaneSet([synth.family((0, 0, 1), 24, 0.8, 40.0, "inverse"), synth.family((0, 1, 0), 5, 0.5, 1.5, "linear")])
+    p_lo = synth.params(5, synth.VAR_FLOOR_U8, 60.0)
+    p_hi = synth.params(7, synth.VAR_FLOOR_U8, 80.0, 0.2, 0.3, 48, 1.1, filters=3)
+    crop = (35, 27, 61, 40)
+    sets = [synth.render_frame(dict(cfg, scene=synth.scene_plane(2.0 + 0.6 * s, (0.5, 2.0), seed=70 + s)), 0) for s in range(3)]
+    masks = [synth.make_mask(128, 96, 80, n_rects=2), None, synth.make_mask(128, 96, 81, n_rects=1)]
+    singles = [oracle.compare.to_numpy(ctx.compute_depth_multires(pl, pc, p_lo, p_hi, crop, st, m, host=True)) for st, m in zip(sets, masks)]
+    outs = ctx.compute_depth_multires_batch(pl, pc, p_lo, p_hi, crop, sets, masks, host=True)
+    for s in range(3):
+        got = oracle.compare.to_numpy(outs[s])
+        for key in ("depth", "best_cost", "second_cost", "plane_index", "valid_reason"):
+            assert np.array_equal(singles[s][key], got[key], equal_nan=True), (s, key)
+    assert (singles[0]["plane_index"] >= 0).sum() > 1000
+    with pytest.raises(fsw.FswError):
+        ctx.compute_depth_multires_batch(pl, pc, p_lo, p_hi, (100, 27, 61, 40), sets, masks, host=True)   # crop leaves the image
+
+
 @pytest.mark.parametrize("idx", [1, 2])
 def test_config_with_filters(idx):
     """C1 / C2 name no filters; SURVEY 8(d) asks for both the raw-valid set and alpha = 0.3/0.3, beta = 1.2."""
