@@ -1,11 +1,13 @@
 #!/usr/bin/env python
 """bench.py -- throughput of the fisheye plane-sweep hot path on B200 (one JSON line on stdout).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C5|C3] [--impl ours|reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C5|C3|P|P3|PH|PM] [--impl ours|reference]
 
 A "step" is one pass of the whole hot path (footprint pack + fused sweep S1..S12) over one synchronized
 frame set of the workload: BASELINE.json configs[4] (C5, the throughput stream: config-3 rig moving 0.5 m per frame,
-192 fronto + 64 ground planes, 9x9 ZNCC, filters and masks on) by default, or configs[2] (C3) with --workload C3.
+192 fronto + 64 ground planes, 9x9 ZNCC, filters and masks on) by default, or configs[2] (C3) with --workload C3, or
+one of the paper's own workload shapes: P = five cameras at full resolution, P3 =
+three of them, PH = half resolution, PM = the multi-scale estimator (fsw_compute_depth_multires_batch).
 `value` = finite (pixel, plane, view) cost evaluations per second, inputs resident in HBM; `e2e` = the same through
 fsw_compute_depth_host (pinned host buffers, copies inside the timed region).  N > 1 (torchrun): frame sets are
 independent, so each rank runs the same number of steps on its own frames -- no data-path collective, "weak".
@@ -29,8 +31,31 @@ import numpy as np  # noqa: E402
 FLOP_PER_EVAL = 70.0   # algorithmic FP32 work of one (pixel, plane, view) cost evaluation
 N_STAGED = 32          # distinct frame sets resident on the device (the C5 stream length)
 METRIC = "plane-sweep cost evals/sec (pixel x plane x view)"
-# dram__bytes_read.sum + dram__bytes_write.sum of one sweep launch, from the committed ncu capture (profiles/)
-NCU_DRAM_BYTES_PER_LAUNCH = {("C5", 8): 156.4e6}
+# dram__bytes_read.sum + dram__bytes_write.sum and issue-slot utilisation of one sweep launch, from the committed ncu
+# captures (profiles/), each with the hash of the kernel source it was taken on (kernel_source_hash()): a figure whose
+# hash no longer matches paper_1809_06132_b200/csrc/fsw_sweep.cuh is reported as null, not as a stale number
+NCU_CAPTURES = {}
+
+
+def kernel_source_hash():
+    import hashlib
+    with open(os.path.join(ROOT, "paper_1809_06132_b200", "csrc", "fsw_sweep.cuh"), "rb") as fh:
+        return hashlib.sha256(fh.read()).hexdigest()[:12]
+
+
+def ncu_capture(workload, batch):
+    cap = NCU_CAPTURES.get((workload, batch))
+    if cap is None or cap["kernel_hash"] != kernel_source_hash():
+        return None
+    return cap
+
+
+def batch_sizes(steps, batch):
+    """`steps` frame sets in ceil(steps / batch) launches of nearly equal size (20 steps, batch 8 -> 7 + 7 + 6): an
+    under-filled last launch would leave the persistent grid unbalanced."""
+    n_calls = max(1, -(-steps // batch))
+    base, extra = divmod(steps, n_calls)
+    return [base + (1 if i < extra else 0) for i in range(n_calls)]
 
 
 def parse_args():
@@ -38,7 +63,7 @@ def parse_args():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=128)
     ap.add_argument("--warmup", type=int, default=8)
-    ap.add_argument("--workload", default="C5", choices=["C5", "C3", "P"])
+    ap.add_argument("--workload", default="C5", choices=["C5", "C3", "P", "P3", "PH", "PM"])
     ap.add_argument("--batch", type=int, default=8,
                     help="frame sets per sweep launch (fsw_compute_depth_batch); 1 = one launch per frame set")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
@@ -49,7 +74,9 @@ def parse_args():
 
 def workload_config(name):
     import synth
-    cfg = synth.make_config({"C5": 5, "C3": 3, "P": 6}[name])
+    if name == "P3":   # the three-camera configuration of PAPER.md:280, :294
+        return synth.make_config(6, cameras=(0, 1, 2))
+    cfg = synth.make_config({"C5": 5, "C3": 3, "P": 6, "PH": 8, "PM": 7}[name])
     if name == "C3":  # the C3 scene, but as a stream of N_STAGED frame sets like C5 so that inputs exceed L2
         cfg = dict(cfg, n_frames=N_STAGED, step_m=0.5, mask_seed=None)
     return cfg
@@ -59,6 +86,15 @@ def workload_label(name):
     if name == "P":
         return ("paper workload shape (PAPER.md:224,249; SURVEY 8(f) 2): 5 fisheye cams (4 matching views, rotated) "
                 "1024x544 u8, 64 fronto + 30 ground planes, 9x9 ZNCC, filters")
+    if name == "P3":
+        return ("paper workload shape, three-camera configuration (PAPER.md:280,294): 3 fisheye cams (2 matching views, "
+                "rotated) 1024x544 u8, 64 fronto + 30 ground planes, 9x9 ZNCC, filters")
+    if name == "PH":
+        return ("paper workload shape at half resolution (PAPER.md:249): 5 fisheye cams 512x272 u8, 64 fronto + 30 ground "
+                "planes, 7x7 ZNCC, filters")
+    if name == "PM":
+        return ("paper workload shape, multi-scale (PAPER.md:88-90,249): 5 fisheye cams 1024x544 u8; 512x272 full field of "
+                "view 7x7 + 572x332 centre crop 9x9, 64 fronto + 30 ground planes in both passes, filters")
     return ("BASELINE.json configs[4]: 32-frame stream, 3 fisheye cams 1280x1024 u8, 192 fronto + 64 ground planes, "
             "9x9 ZNCC, filters + masks" if name == "C5" else
             "BASELINE.json configs[2]: 3 fisheye cams 1280x1024 u8, 96 fronto + 32 ground planes, 9x9 ZNCC, filters")
@@ -127,16 +163,30 @@ def cropped_rig(cfg, crop_w, crop_h):
     return cams, (x0, y0)
 
 
-def oracle_sample(cfg, frame_images, mask, crop_w, crop_h):
-    """Runs the oracle as it stands on a centred crop; returns (seconds, n_eval)."""
+def is_multires(cfg):
+    return "families_low" in cfg
+
+
+def oracle_sample(cfg, frame_images, mask, crop_w, crop_h, keep=False):
+    """Runs the oracle as it stands on a centred crop_w x crop_h window of the frame set (the whole frame set when the
+    window is the image); returns (seconds, n_eval, maps)."""
     import oracle
     cams, (x0, y0) = cropped_rig(cfg, crop_w, crop_h)
     imgs = [np.ascontiguousarray(im[y0:y0 + crop_h, x0:x0 + crop_w]) for im in frame_images]
     m = None if mask is None else np.ascontiguousarray(mask[y0:y0 + crop_h, x0:x0 + crop_w])
-    params = dict(cfg["params"], horizon_row=cfg["params"]["horizon_row"] - y0)
     t0 = time.perf_counter()
-    out = oracle.compute_depth(cams, cfg["ref_index"], cfg["families"], params, imgs, m)
-    return time.perf_counter() - t0, int(out["n_eval"])
+    if is_multires(cfg):
+        pl = dict(cfg["params_low"], horizon_row=cfg["params_low"]["horizon_row"] - y0)
+        pc = dict(cfg["params_crop"], horizon_row=cfg["params_crop"]["horizon_row"] - y0)
+        cx0, cy0, cw, ch = cfg["crop"]   # the crop of the multi-scale pass, clipped to the sampled window
+        ax0, ay0 = max(cx0 - x0, 0), max(cy0 - y0, 0)
+        ax1, ay1 = min(cx0 + cw - x0, crop_w), min(cy0 + ch - y0, crop_h)
+        out = oracle.compute_depth_multires(cams, cfg["ref_index"], cfg["families_low"], cfg["families_crop"], pl, pc,
+                                            (ax0, ay0, ax1 - ax0, ay1 - ay0), imgs, m, keep_cost=keep)
+    else:
+        params = dict(cfg["params"], horizon_row=cfg["params"]["horizon_row"] - y0)
+        out = oracle.compute_depth(cams, cfg["ref_index"], cfg["families"], params, imgs, m, keep_cost=keep)
+    return time.perf_counter() - t0, int(out["n_eval"]), out
 
 
 def run_reference(args, rank):
@@ -150,7 +200,7 @@ def run_reference(args, rank):
     total_steps = args.steps + args.warmup
     # size the crop so that the whole run stays within a few minutes (oracle ~ 1e7 evals/s per 8 cores)
     budget_s = 150.0
-    planes_views = sum(f["n_planes"] for f in cfg["families"]) * (len(cfg["cams"]) - 1)
+    planes_views = sum(f["n_planes"] for f in cfg.get("families", cfg.get("families_crop"))) * (len(cfg["cams"]) - 1)
     est_rate = 1.2e6 * max(oracle.num_threads(), 1)
     px = max(48 * 36, int(budget_s / max(total_steps, 1) * est_rate / planes_views))
     crop_h = int(min(640, max(36, (px / (4.0 / 3.0)) ** 0.5))) // 4 * 4
@@ -162,7 +212,7 @@ def run_reference(args, rank):
         if f not in frames:
             frames[f] = synth.render_frame(cfg, f)
         mask = None if cfg.get("mask_seed") is None else synth.make_mask(cfg["cams"][0]["width"], cfg["cams"][0]["height"], cfg["mask_seed"] + f)
-        dt, ne = oracle_sample(cfg, frames[f], mask, crop_w, crop_h)
+        dt, ne, _ = oracle_sample(cfg, frames[f], mask, crop_w, crop_h)
         if s >= args.warmup:
             times.append(dt)
             evals.append(ne)
@@ -209,7 +259,14 @@ def run_ours(args, rank, local_rank, world):
     dev_frames = [[torch.from_numpy(im).to(dev) for im in fr] for fr in host_frames]
     dev_masks = [torch.from_numpy(m).to(dev) for m in host_masks] or [None] * N_STAGED
     rig = fsw.Rig(cfg["cams"], cfg["ref_index"])
-    planes = fsw.PlaneSet(cfg["families"])
+    multires = is_multires(cfg)
+    if multires:
+        planes_low, planes = fsw.PlaneSet(cfg["families_low"]), fsw.PlaneSet(cfg["families_crop"])
+        n_nominal = (W // 2) * (H // 2) * planes_low.n_planes * (rig.n_cams - 1) + \
+            cfg["crop"][2] * cfg["crop"][3] * planes.n_planes * (rig.n_cams - 1)
+    else:
+        planes = fsw.PlaneSet(cfg["families"])
+        n_nominal = W * H * planes.n_planes * (rig.n_cams - 1)
     ctx = fsw.Context(rig, local_rank)
     # every frame set gets its own output maps so that the bytes touched per pass exceed the 126 MB L2
     outs = [dict(depth=torch.empty((H, W), dtype=torch.float32, device=dev),
@@ -220,36 +277,45 @@ def run_ours(args, rank, local_rank, world):
 
     B = max(1, min(args.batch, N_STAGED))
 
+    def call_one(c, images, mask, out, host=False):
+        """one frame set per call: fsw_compute_depth(_host) or fsw_compute_depth_multires(_host)"""
+        if multires:
+            return c.compute_depth_multires(planes_low, planes, cfg["params_low"], cfg["params_crop"], cfg["crop"], images,
+                                            mask, host=host, out=out)
+        return c.compute_depth(planes, cfg["params"], images, mask, host=host, out=out)
+
+    def call_batch(c, image_sets, masks, outs_, host=False, want=fsw.Context.ALL):
+        """several frame sets per call: fsw_compute_depth_batch(_host) or fsw_compute_depth_multires_batch(_host)"""
+        if multires:
+            return c.compute_depth_multires_batch(planes_low, planes, cfg["params_low"], cfg["params_crop"], cfg["crop"],
+                                                  image_sets, masks, want=want, host=host, outs=outs_)
+        return c.compute_depth_batch(planes, cfg["params"], image_sets, masks, want=want, host=host, outs=outs_)
+
     def step(i):
         f = i % N_STAGED
-        ctx.compute_depth(planes, cfg["params"], dev_frames[f], dev_masks[f], out=outs[f])
+        call_one(ctx, dev_frames[f], dev_masks[f], outs[f])
 
     def run_steps(first, n, host=False):
-        """steps first .. first+n-1, B consecutive frame sets per launch (the stream is processed in order).
-        host: through the *_host calls, alternating between two contexts on two streams (fsw_context_set_host_async)
-        so that the copies of one batch overlap the sweep of the other; every batch still does its own host-to-device
-        copies, kernels and device-to-host copy of the depth maps, in that order, on its stream."""
+        """steps first .. first+n-1 in launches of nearly equal size, at most B consecutive frame sets each (the stream
+        is processed in order).  host: through the *_host calls, alternating between two contexts on two streams
+        (fsw_context_set_host_async) so that the copies of one batch overlap the sweep of the other; every batch still
+        does its own host-to-device copies, kernels and device-to-host copy of the depth maps, in that order, on its
+        stream."""
         i = first
-        call = 0
-        while i < first + n:
-            nb = min(B, first + n - i)
+        for call, nb in enumerate(batch_sizes(n, B)):
             fs = [(i + j) % N_STAGED for j in range(nb)]
             if host:
                 lane = call % 2
                 with torch.cuda.stream(e2e_streams[lane]):
                     if nb == 1:
-                        e2e_ctx[lane].compute_depth(planes, cfg["params"], pin_frames[fs[0]], pin_masks[fs[0]], host=True,
-                                                    out=pin_outs[lane][0])
+                        call_one(e2e_ctx[lane], pin_frames[fs[0]], pin_masks[fs[0]], pin_outs[lane][0], host=True)
                     else:
-                        e2e_ctx[lane].compute_depth_batch(planes, cfg["params"], [pin_frames[f] for f in fs],
-                                                          [pin_masks[f] for f in fs], want=("depth",), host=True,
-                                                          outs=pin_outs[lane][:nb])
-                call += 1
+                        call_batch(e2e_ctx[lane], [pin_frames[f] for f in fs], [pin_masks[f] for f in fs],
+                                   pin_outs[lane][:nb], host=True, want=("depth",))
             elif nb == 1:
                 step(i)
             else:
-                ctx.compute_depth_batch(planes, cfg["params"], [dev_frames[f] for f in fs], [dev_masks[f] for f in fs],
-                                        outs=[outs[f] for f in fs])
+                call_batch(ctx, [dev_frames[f] for f in fs], [dev_masks[f] for f in fs], [outs[f] for f in fs])
             i += nb
 
     def barrier():
@@ -278,18 +344,20 @@ def run_ours(args, rank, local_rank, world):
     sampler.stop_flag = True
     barrier()
     ms_total = ev0.elapsed_time(ev1)
-    launches_per_step = ctx.last_counters()["n_launches"]  # kernels of one call of the timed loop (B frame sets)
-    n_calls = (args.steps + B - 1) // B
+    launches_per_step = ctx.last_counters()["n_launches"]  # kernels of one call of the timed loop
+    sizes = batch_sizes(args.steps, B)                      # frame sets per call of the timed loop
+    n_calls = len(sizes)
+    Bt = sizes[0]
     launches = launches_per_step * n_calls
     evals_total = float(sum(n_eval_step[i % len(n_eval_step)] for i in range(args.steps)))
 
     # ---- the sweep kernel alone: CUDA events around its launches on the same stream (fsw_context_set_timing) ------
     ctx.set_timing(True)
     sweep_ms, sweep_evals = [], []
-    for i in range(0, min(args.steps, 2 * N_STAGED) // B * B, B):
-        run_steps(i, B)
+    for i in range(0, max(Bt, min(args.steps, 2 * N_STAGED) // Bt * Bt), Bt):   # launches of the size the timed loop used
+        run_steps(i, Bt)
         sweep_ms.append(ctx.last_counters()["sweep_ms"])
-        sweep_evals.append(sum(n_eval_step[(i + j) % len(n_eval_step)] for j in range(B)))
+        sweep_evals.append(sum(n_eval_step[(i + j) % len(n_eval_step)] for j in range(Bt)))
     ctx.set_timing(False)
     sweep_ms_avg = float(np.mean(sweep_ms))
     evals_per_launch = float(np.mean(sweep_evals))
@@ -314,7 +382,7 @@ def run_ours(args, rank, local_rank, world):
     for c in e2e_ctx:
         c.set_host_async(True)
 
-    run_steps(0, 4 * B, host=True)
+    run_steps(0, min(4 * B, N_STAGED), host=True)
     e2e_steps = args.steps
     barrier()
     ev0.record(stream)
@@ -340,60 +408,89 @@ def run_ours(args, rank, local_rank, world):
         value = evals_all / (ms_total * 1e-3)
         e2e_value = evals_all / (ms_e2e * 1e-3)
         achieved = evals_per_launch * FLOP_PER_EVAL / (sweep_ms_avg * 1e-3) / 1e12
+        cap = ncu_capture(args.workload, Bt)
+        n_cam_bytes = sum(int(t.numel() * t.element_size()) for t in dev_frames[0])
         line = {
             "metric": METRIC, "value": value, "unit": "evals/s", "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f32", "data": "synthetic",
             "config": {"workload": workload_label(args.workload), "frames_staged_per_gpu": N_STAGED,
-                       "n_eval_per_step": evals_total / args.steps, "n_nominal_per_step": W * H * planes.n_planes * (rig.n_cams - 1),
-                       "l2": "inputs and outputs rotate over %d distinct frame sets (%.0f MB per pass) > 126 MB L2" % (
-                           N_STAGED, N_STAGED * (3 * W * H + W * H + W * H * 15 + 2 * W * H * 4) / 1e6),
-                       "frame_sets_per_launch": B, "ms_single_frame_set_launch": ms_single,
+                       "n_eval_per_step": evals_total / args.steps, "n_nominal_per_step": n_nominal,
+                       "l2": "inputs, footprint images and outputs rotate over %d distinct frame sets (%.0f MB per pass) "
+                             "> 126 MB L2" % (N_STAGED, N_STAGED * (n_cam_bytes * 9 + W * H + W * H * 15) / 1e6),
+                       "frame_sets_per_launch": sizes, "ms_single_frame_set_launch": ms_single,
                        "parallelism": "frame sets sharded over %d GPU(s), no collective" % world},
-            "depth_maps_per_s": world * args.steps / (ms_total * 1e-3) if dist is None else None,
+            "depth_maps_per_s": world * args.steps / (ms_total * 1e-3),
+            # what a real-time pipeline sees: one frame set per call (25 frame sets per second arrive)
+            "single_frame_set": {"ms_per_map": ms_single, "depth_maps_per_s": 1e3 / ms_single,
+                                 "evals_per_s": evals_total / args.steps / (ms_single * 1e-3)},
             "clocks": sampler.summary(),
             "e2e": {"value": e2e_value, "unit": "evals/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "ms_per_step": ms_e2e / e2e_steps, "depth_maps_per_s": world * e2e_steps / (ms_e2e * 1e-3),
-                    "how": "fsw_compute_depth_batch_host on pinned host buffers: every batch copies its images and masks "
+                    "how": "fsw_compute_depth_%sbatch_host on pinned host buffers: every batch copies its images and masks "
                            "to the device, runs the kernels and copies its depth maps back, on one of two streams "
-                           "(two contexts, fsw_context_set_host_async) so that copies overlap the other batch's sweep"},
+                           "(two contexts, fsw_context_set_host_async) so that copies overlap the other batch's sweep"
+                           % ("multires_" if multires else "")},
             "gpu_launches": launches,
             "roofline": {"bound": "alu", "achieved": achieved, "peak": fp32_tflops, "unit": "TFLOP/s",
                          "frac": achieved / fp32_tflops if fp32_tflops else None,
-                         "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get((args.workload, B)),
-                         "traffic_source": "profiles/r1_launches_c5_v6.md (ncu --set full, dram bytes read + written by "
-                                           "one sweep launch)" if (args.workload, B) in NCU_DRAM_BYTES_PER_LAUNCH else None,
-                         "ncu_issue_active_pct": 65.6 if (args.workload, B) in NCU_DRAM_BYTES_PER_LAUNCH else None,
-                         "frame_sets_per_launch": B, "evals_per_launch": evals_per_launch,
-                         "kernel": "fsw::sweep_kernel<9,...>", "kernel_ms": sweep_ms_avg,
+                         "traffic": cap["dram_bytes"] if cap else None,
+                         "traffic_source": cap["source"] if cap else None,
+                         "ncu_issue_active_pct": cap["issue_active_pct"] if cap else None,
+                         "ncu_fma_pipe_pct": cap["fma_pipe_pct"] if cap else None,
+                         "ncu_alu_pipe_pct": cap["alu_pipe_pct"] if cap else None,
+                         "kernel_source_hash": kernel_source_hash(),
+                         "frame_sets_per_launch": Bt, "evals_per_launch": evals_per_launch,
+                         "kernel": "fsw::sweep_kernel<%d,...>%s" % (
+                             cfg.get("params", cfg.get("params_crop"))["window"],
+                             " (both sweeps of the multi-scale call)" if multires else ""),
+                         "kernel_ms": sweep_ms_avg,
                          "flop_per_eval": FLOP_PER_EVAL,
                          "peak_source": "FFMA-chain kernel measured in this run (MEASURED_PEAKS.json has no FP32 figure); "
                                         "nominal 148 SM x 128 lanes x 2 x clock"},
         }
-        line["depth_maps_per_s"] = world * args.steps / (ms_total * 1e-3)
         if not args.no_cpu_baseline:
-            line["cpu_baseline"] = cpu_baseline(cfg, host_frames, host_masks, args.cpu_baseline_seconds)
+            step(0)
+            torch.cuda.synchronize()
+            gpu0 = {k: v.cpu().numpy() for k, v in outs[0].items()}
+            line["cpu_baseline"], line["parity"] = cpu_baseline(cfg, host_frames, host_masks, args.cpu_baseline_seconds, gpu0)
         print(json.dumps(line), flush=True)
     if dist is not None:
         dist.barrier()
         dist.destroy_process_group()
 
 
-def cpu_baseline(cfg, frames, masks, seconds):
+def cpu_baseline(cfg, frames, masks, seconds, gpu_maps0=None):
     """The oracle as it stands, timed on this box's host cores on a bounded sample of the workload: whole frame sets
-    of the stream (every plane and view), one after the other, until `seconds` of CPU work are done (at most 6)."""
+    of the stream (every plane and view), one after the other, until `seconds` of CPU work are done (at most 6).
+    The oracle's maps of frame set 0 are also held against the GPU's (oracle/compare.py): the parity statistics of
+    this very run go into the bench line."""
     import oracle
+    from oracle.compare import compare_maps, depth_conditioning
     oracle.build()
     cores = oracle.num_threads()
     W, H = cfg["cams"][0]["width"], cfg["cams"][0]["height"]
     total_t, total_e, n = 0.0, 0, 0
+    parity = None
     while n < min(6, len(frames)) and total_t < seconds:
-        dt, ne = oracle_sample(cfg, frames[n], masks[n] if masks else None, W, H)
+        dt, ne, maps = oracle_sample(cfg, frames[n], masks[n] if masks else None, W, H, keep=(n == 0 and gpu_maps0 is not None))
+        if n == 0 and gpu_maps0 is not None:
+            if is_multires(cfg):
+                st = compare_maps(maps, gpu_maps0, (maps["cost_lo"], maps["cost_hi"]))
+            else:
+                cond = depth_conditioning(maps, oracle.plane_table(cfg["families"])[0])
+                st = compare_maps(maps, gpu_maps0, maps["cost"], depth_cond=cond)
+            keys = ("index_exact_frac", "index_match_frac", "max_dc1", "max_dc2", "frac_ddepth_over_tol",
+                    "depth_worst_ratio_to_bound", "fragile_frac", "valid_mismatch_nonfragile", "n_oracle_valid")
+            parity = {k: st[k] for k in keys}
+            parity["frame_set"] = 0
+            maps = None
         total_t += dt
         total_e += ne
         n += 1
-    return {"value": total_e / total_t, "unit": "evals/s", "cores": cores, "kind": "oracle", "seconds": total_t,
+    base = {"value": total_e / total_t, "unit": "evals/s", "cores": cores, "kind": "oracle", "seconds": total_t,
             "sample": "frame sets 0..%d of the workload at full size (%dx%d), all planes and views" % (n - 1, W, H)}
+    return base, parity
 
 
 def main():
