@@ -271,6 +271,8 @@ int32_t check_out(const fsw_rig& rig, const fsw_depth_out* out, const uint8_t* m
     return FSW_OK;
 }
 
+bool view_fov_inside_image(const fsw_camera& c, bool half);
+
 /* fills the part of the argument block that depends on rig, planes and parameters */
 int32_t fill_args(FswSweepArgs& a, const fsw_rig& rig, const fsw_planeset& ps, const fsw_sweep_params& p, bool half) {
     std::memset(&a, 0, sizeof(a));
@@ -278,6 +280,7 @@ int32_t fill_args(FswSweepArgs& a, const fsw_rig& rig, const fsw_planeset& ps, c
     a.ref = dev_cam(ref, half);
     a.ref_rd2_max = ref_rd2_bound(ref); /* normalised coordinates: the same at both resolutions */
     a.n_views = 0;
+    bool inside = true;
     for (int c = 0; c < rig.n_cams; ++c) {
         if (c == rig.ref_index) continue;
         FswDevView& v = a.views[a.n_views++];
@@ -289,7 +292,9 @@ int32_t fill_args(FswSweepArgs& a, const fsw_rig& rig, const fsw_planeset& ps, c
         }
         for (int i = 0; i < 3; ++i) v.T[i] = (float)rig.Trel[c][i];
         v.ident_R = ident ? 1 : 0;
+        inside = inside && view_fov_inside_image(rig.cams[c], half);
     }
+    a.views_inside = inside ? 1 : 0;
     a.n_fams = ps.n_fams;
     a.n_planes = ps.n_planes;
     for (int f = 0; f < ps.n_fams; ++f) {
@@ -345,7 +350,22 @@ int pick_variant(const FswSweepArgs& a, int foot_f16) {
         simple = simple && (a.views[v].cam.cos_fov_xi >= 1e-3f); /* lets the kernel drop the denominator test */
     }
     const int mode = !simple ? 0 : (ident ? 1 : 2);
+    if (mode != 0 && foot_f16 && a.views_inside) return 5 + mode; /* 6, 7: no test against the image borders */
     return mode + (foot_f16 ? 3 : 0);
+}
+
+/* Does the whole field of view of the camera fall inside its raster, with half a pixel to spare on every side?  Then
+ * a projection that passes the field-of-view test has its bilinear footprint inside the image (S3) and the kernel
+ * drops the border test.  Only where the edge of the field of view is a provable bound of the distorted radius
+ * (ref_rd2_bound: radial distortion only, monotone, 2 % margin included). */
+bool view_fov_inside_image(const fsw_camera& c, bool half) {
+    const float rd2 = ref_rd2_bound(c);
+    if (!std::isfinite(rd2)) return false;
+    const double rd = std::sqrt((double)rd2);
+    const FswDevCam d = dev_cam(c, half);
+    const double rx = (double)d.fx * rd, ry = (double)d.fy * rd;
+    return (double)d.cx - rx >= 0.5 && (double)d.cx + rx <= (double)d.W - 1.5 &&
+           (double)d.cy - ry >= 0.5 && (double)d.cy + ry <= (double)d.H - 1.5;
 }
 
 /* Scheduling order of the tiles (S0): nearest to the principal point first, lower image half before the upper
@@ -457,7 +477,7 @@ int32_t launch_sweep(fsw_context* ctx, FswSweepArgs& a, int w, cudaStream_t s) {
     auto launch_one = [&](const FswSweepArgs& la, cudaStream_t ls) -> cudaError_t {
         const long long items = la.split ? 2LL * la.slot_count - la.split_whole : (long long)la.n_tiles * la.n_sets;
         const int grid = (int)(items < slots ? items : slots);
-        const int var = pick_variant(la, la.foot_f16) + (la.split ? 6 : 0);
+        const int var = pick_variant(la, la.foot_f16) + (la.split ? 8 : 0);
         return fsw_launch_sweep(w, la, var, grid, ls);
     };
     a.slot_first = 0;

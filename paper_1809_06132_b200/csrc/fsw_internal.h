@@ -100,6 +100,7 @@ struct FswSweepArgs {
                             (+inf when the bound does not apply): tiles entirely beyond it skip S1 */
     int32_t lo_W, lo_H;
     int32_t foot_f16;   /* 1: the footprint images hold four bfloat16 per pixel, 0: four floats */
+    int32_t views_inside; /* 1: the field of view of every view lies inside its image (no border test needed) */
     int32_t index_flag; /* OR-ed into the plane index this pass writes (FSW_INDEX_FROM_CROP or 0) */
     /* frame sets: set0 inline for the single-set calls, `sets` (device array) for batches */
     int32_t n_sets;

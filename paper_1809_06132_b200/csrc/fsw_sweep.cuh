@@ -77,12 +77,15 @@ struct Geo {
      * second set of row-sum planes brings the block to 203 KB of the 227 KB an sm_100 block may use (the footprint
      * gathers then have 28 KB of L1 instead of 88 KB: measured + 4 % on the unfused kernel, against - 12 % from fusing) */
     static constexpr bool FUSE_OK = A_IN_REGS;
+    /* the parabola neighbours of the running best in shared memory instead of registers (Wta::update): where the
+     * block has the 20 KB to spare */
+    static constexpr bool NBR_SMEM = WIN <= 9;
     static_assert(EH <= EHA && TX % 32 == 0 && TX % RUN == 0 && NRUN == 8, "tile / thread mapping");
     static_assert(SB >= SBMIN && SB % 4 == 0 && HS % 8 == 4, "aligned strides");
     static_assert(R * NRUN <= 32, "one horizontal work item per lane");
     static constexpr size_t smem(bool fuse) {
         return sizeof(float4) * PLANE + sizeof(float) * ((size_t)2 * PLANE + (size_t)(fuse ? 8 : 4) * HPLANE) +
-               sizeof(float2) * TX * TY;
+               (NBR_SMEM ? 2 : 1) * sizeof(float2) * TX * TY;
     }
 };
 
@@ -163,13 +166,15 @@ __device__ inline bool back_project(const FswDevCam& c, float u, float v, float&
  * intersection is beyond range_max: the NaN then fails the field-of-view test below, no separate flag is carried).
  * IDENT: the view's relative rotation is the identity.  FULLDIST: k2 / p1 / p2 may be non-zero.
  * CHECKDEN: cos(fov/2) + xi may be < 1e-3, so the projection denominator is tested on its own.
+ * INSIDE: the image circle of every view lies inside its raster with half a pixel to spare (decided on the host,
+ *   fsw_api.cu: view_fov_inside_image), so a sample inside the field of view needs no test against the image borders.
  * F16: the footprint images hold four bfloat16 per pixel (8-bit views) instead of four floats. */
 struct SampleAddr {
     float au, av;  /* bilinear weights */
     unsigned idx;  /* footprint index iy * W + ix, 0 for an invalid sample */
     bool ok;
 };
-template <bool IDENT, bool FULLDIST, bool CHECKDEN>
+template <bool IDENT, bool FULLDIST, bool CHECKDEN, bool INSIDE>
 __device__ __forceinline__ SampleAddr sample_addr(float rx, float ry, float rz, float s, const FswDevView& k) {
     /* S2: X' ~ R r + s T */
     float X, Y, Z;
@@ -208,7 +213,7 @@ __device__ __forceinline__ SampleAddr sample_addr(float rx, float ry, float rz, 
     float tu = __fadd_rd(u, 12582912.f), tv = __fadd_rd(v, 12582912.f);
     unsigned ix = (unsigned)__float_as_int(tu) - 0x4B400000u, iy = (unsigned)__float_as_int(tv) - 0x4B400000u;
     /* bilinear footprint inside the view image: 0 <= u < W-1, 0 <= v < H-1  <=>  0 <= floor(u) < W-1, ... */
-    ok = ok && (ix < (unsigned)k.cam.Wm1) && (iy < (unsigned)k.cam.Hm1);
+    if (!INSIDE) ok = ok && (ix < (unsigned)k.cam.Wm1) && (iy < (unsigned)k.cam.Hm1);
     SampleAddr a;
     a.au = u - (tu - 12582912.f);
     a.av = v - (tv - 12582912.f);
@@ -373,16 +378,18 @@ struct Wta {
     /* Planes are visited in ascending index order (dir = +1), or -- in the second half of a split tile -- in
      * descending order (dir = -1, desc): then an equal cost wins as well (the later plane has the lower index), and
      * cm / cp hold the neighbour visited before / after the best, i.e. above / below it (swap_neighbours()). */
+    /* During the sweep the two neighbours of the best live in shared memory (*nbr = (cm, cp), written by this thread
+     * only): they change when a new best arrives or the plane after it is scored, which is rare, and ten registers
+     * fewer let the sample phase keep more footprint fetches in flight. */
     template <bool KNEXT>
-    __device__ __forceinline__ void update(float c, int k, int dir, bool desc, bool fam_first) {
+    __device__ __forceinline__ void update(float c, int k, int dir, bool desc, bool fam_first, float2* __restrict__ nbr) {
         /* neighbour of the running best on the far side (same family): not eligible as second best */
         const bool isn = KNEXT ? (k == knext) : (!fam_first && (k == k1 + dir));
         const bool nb = desc ? ((c <= b1) && (c < CUDART_INF_F)) : (c < b1); /* lowest index wins ties */
-        cp = isn ? c : cp;
+        if (isn) nbr->y = c;
         const float t = isn ? s2 : fminf(s2, c);
         s2 = nb ? m2 : t;
-        cm = nb ? cprev : cm;
-        cp = nb ? CUDART_INF_F : cp;
+        if (nb) *nbr = make_float2(cprev, CUDART_INF_F);
         k1 = nb ? k : k1;
         if (KNEXT) knext = nb ? k + dir : knext;
         m2 = b1;
@@ -415,59 +422,52 @@ __device__ __forceinline__ void h_item(int lane, int& row, int& run) {
 /* S2-S4 for the R halo rows of one warp, one plane and NJ views (1 or 2): samples into the warp's rows of b0 (first
  * view) and b1 (second view), NaN = invalid.  The ray, its inverse range s = (n.r)/d_k and the range test are shared by
  * the views.  Returns (warp-uniform) bit j set iff every sample of the rows is valid in view j. */
-template <class G, int NJ, bool IDENT, bool FULLDIST, bool CHECKDEN, bool F16>
+template <class G, int NJ, bool IDENT, bool FULLDIST, bool CHECKDEN, bool INSIDE, bool F16>
 __device__ __forceinline__ unsigned sample_rows(const float4* __restrict__ rays, float* __restrict__ b0, float* __restrict__ b1,
                                                 int sbase, bool tail_on, float inv_d, float s_min,
                                                 const FswDevView& view0, const FswDevView& view1,
                                                 const void* __restrict__ f0, const void* __restrict__ f1, float centre) {
     constexpr int NS = G::NS;
-    /* samples in flight per lane: four with the 8-byte footprints of the specialised variants, two otherwise (the raw
-     * footprints of a batch stay in registers); a batch is SLOTS halo pixels x NJ views */
-    constexpr int SLOTS = ((!FULLDIST && F16) ? 4 : 2) / NJ;
+    /* Samples in flight per lane: four with the 8-byte footprints of the specialised variants, two otherwise (the raw
+     * footprints stay in registers).  The slots (one halo pixel x NJ views each) run through a software pipeline of
+     * DEPTH stages: the addresses and footprint fetches of slot i + DEPTH - 1 are issued before the lerps of slot i, so
+     * that a fetch that misses L1 has a whole slot of arithmetic to come back from L2.  An invalid sample carries a
+     * NaN weight au (and fetches footprint 0 instead of branching), so its lerp yields the NaN that marks it in the
+     * sample plane. */
+    constexpr int DEPTH = (((!FULLDIST && F16) ? 4 : 2) / NJ) > 1 ? 3 : 1;
     bool all_ok[NJ];
 #pragma unroll
     for (int v = 0; v < NJ; ++v) all_ok[v] = true;
-    /* batches: all addresses, then all fetches, then the lerps.  An invalid sample carries a NaN weight au (and
-     * fetches footprint 0 instead of branching), so its lerp yields the NaN that marks it in the sample plane. */
+    float au[DEPTH][NJ], av[DEPTH][NJ];
+    FootRaw<F16> raw[DEPTH][NJ];
+    auto issue = [&](const int i) { /* S2-S3 + the fetch of S4 for slot i */
+        const int st = i % DEPTH;
+        const float4 ry = rays[sbase + 32 * i];
+        float s = ry.w * inv_d;
+        s = (s >= s_min) ? s : CUDART_NAN_F;
 #pragma unroll
-    for (int i0 = 0; i0 < NS; i0 += SLOTS) {
-        float au[SLOTS][NJ], av[SLOTS][NJ];
-        unsigned idx[SLOTS][NJ];
-        FootRaw<F16> raw[SLOTS][NJ];
-#pragma unroll
-        for (int jj = 0; jj < SLOTS; ++jj) {
-            const int i = i0 + jj;
-#pragma unroll
-            for (int v = 0; v < NJ; ++v) { au[jj][v] = 0.f; av[jj][v] = 0.f; idx[jj][v] = 0u; }
-            if (i < NS) {
-                const float4 ry = rays[sbase + 32 * i];
-                float s = ry.w * inv_d;
-                s = (s >= s_min) ? s : CUDART_NAN_F;
-#pragma unroll
-                for (int v = 0; v < NJ; ++v) {
-                    SampleAddr a = sample_addr<IDENT, FULLDIST, CHECKDEN>(ry.x, ry.y, ry.z, s, v ? view1 : view0);
-                    const bool on = a.ok && (i < G::NSFULL || tail_on); /* a pixel in this slot */
-                    au[jj][v] = on ? a.au : CUDART_NAN_F; av[jj][v] = a.av;
-                    idx[jj][v] = on ? a.idx : 0u;
-                    if (i < G::NSFULL || tail_on) all_ok[v] = all_ok[v] && on;
-                }
-            }
+        for (int v = 0; v < NJ; ++v) {
+            SampleAddr a = sample_addr<IDENT, FULLDIST, CHECKDEN, INSIDE>(ry.x, ry.y, ry.z, s, v ? view1 : view0);
+            const bool on = a.ok && (i < G::NSFULL || tail_on); /* a pixel in this slot */
+            au[st][v] = on ? a.au : CUDART_NAN_F; av[st][v] = a.av;
+            if (i < G::NSFULL || tail_on) all_ok[v] = all_ok[v] && on;
+            raw[st][v] = foot_fetch<F16>(v ? f1 : f0, on ? a.idx : 0u);
         }
+    };
+    auto finish = [&](const int i) { /* the lerp of S4 for slot i */
+        const int st = i % DEPTH;
 #pragma unroll
-        for (int jj = 0; jj < SLOTS; ++jj)
-#pragma unroll
-            for (int v = 0; v < NJ; ++v)
-                if (i0 + jj < NS) raw[jj][v] = foot_fetch<F16>(v ? f1 : f0, idx[jj][v]);
-#pragma unroll
-        for (int jj = 0; jj < SLOTS; ++jj) {
-            const int i = i0 + jj;
-#pragma unroll
-            for (int v = 0; v < NJ; ++v)
-                if (i < NS) {
-                    const float b = foot_lerp<F16>(raw[jj][v], au[jj][v], av[jj][v], centre);
-                    if (i < G::NSFULL || tail_on) (v ? b1 : b0)[sbase + 32 * i] = b;
-                }
+        for (int v = 0; v < NJ; ++v) {
+            const float b = foot_lerp<F16>(raw[st][v], au[st][v], av[st][v], centre);
+            if (i < G::NSFULL || tail_on) (v ? b1 : b0)[sbase + 32 * i] = b;
         }
+    };
+#pragma unroll
+    for (int i = 0; i < DEPTH - 1; ++i) issue(i);
+#pragma unroll
+    for (int i = 0; i < NS; ++i) {
+        if (i + DEPTH - 1 < NS) issue(i + DEPTH - 1);
+        finish(i);
     }
     unsigned m = __all_sync(0xffffffffu, all_ok[0]) ? 1u : 0u;
     if (NJ > 1) m |= __all_sync(0xffffffffu, all_ok[NJ - 1]) ? 2u : 0u;
@@ -482,7 +482,7 @@ struct SetHot {
 
 /* NVT = number of views known at compile time (1..4), 0 = read args.n_views at run time (then the view parameters
  * come from a copy in shared memory, not from dynamically indexed kernel parameters). */
-template <int WIN, int NVT, bool IDENT, bool FULLDIST, bool CHECKDEN, bool F16, bool SPLIT>
+template <int WIN, int NVT, bool IDENT, bool FULLDIST, bool CHECKDEN, bool INSIDE, bool F16, bool SPLIT>
 __global__ void __launch_bounds__(Geo<WIN>::NT, 1) sweep_kernel(const __grid_constant__ FswSweepArgs args) {
     using G = Geo<WIN>;
     constexpr int HW = G::HW, RPT = G::RPT, NS = G::NS, TX = G::TX, TY = G::TY, R = G::R;
@@ -510,6 +510,8 @@ __global__ void __launch_bounds__(Geo<WIN>::NT, 1) sweep_kernel(const __grid_con
     const int col = tid % TX, grp = tid / TX;
     /* [TY][TX]: reference-side window statistics of every output: ((sum a')/N, sum a'^2 - (sum a')^2/N) */
     float2* const a_stat = reinterpret_cast<float2*>(hs + NJ * 4 * G::HPLANE) + (grp * RPT) * TX + col;
+    /* [TY][TX]: costs of the planes below / above the running best of every output (Wta::update) */
+    float2* const nbr_s = a_stat + TX * TY;
     const int W = args.ref.W, H = args.ref.H;
     /* split launches: the first split_whole (tile, set) slots are swept whole, every later one as two halves */
     /* a split launch covers the (tile, set) slots slot_first .. slot_first + slot_count - 1 of the queue order, an
@@ -560,8 +562,13 @@ __global__ void __launch_bounds__(Geo<WIN>::NT, 1) sweep_kernel(const __grid_con
         const int oy0 = y0t + grp * RPT;     /* ... and first output row */
 
         Wta st[RPT];
+        float2 nbr_r[G::NBR_SMEM ? 1 : RPT]; /* ... or in registers */
+        auto nbr_at = [&](const int i) -> float2* { return G::NBR_SMEM ? &nbr_s[i * TX] : &nbr_r[G::NBR_SMEM ? 0 : i]; };
 #pragma unroll
-        for (int i = 0; i < RPT; ++i) st[i].init();
+        for (int i = 0; i < RPT; ++i) {
+            st[i].init();
+            *nbr_at(i) = make_float2(CUDART_INF_F, CUDART_INF_F);
+        }
         unsigned n_eval = 0;
 
         bool tile_live = (x0t < args.roi_x1) && (x0t + TX > args.roi_x0) && (y0t < args.roi_y1) && (y0t + TY > args.roi_y0);
@@ -731,7 +738,7 @@ __global__ void __launch_bounds__(Geo<WIN>::NT, 1) sweep_kernel(const __grid_con
                             /* ---- S2-S4: sample the plane-warped views at this warp's halo rows ----------------- */
                             unsigned okmask = (1u << NJP) - 1u;
                             if (rows_on)
-                                okmask = sample_rows<G, NJP, IDENT, FULLDIST, CHECKDEN, F16>(
+                                okmask = sample_rows<G, NJP, IDENT, FULLDIST, CHECKDEN, INSIDE, F16>(
                                     rays, b0, bs1, sbase, tail_on, inv_d, args.inv_range_max, vw0, vw1,
                                     s_set.foot[va], s_set.foot[vb], centre);
                             __syncwarp();
@@ -836,10 +843,10 @@ __global__ void __launch_bounds__(Geo<WIN>::NT, 1) sweep_kernel(const __grid_con
                         else c = ci == n_views ? acc[i] * inv_views : acc[i] * args.inv_count[ci];
                         c = ci > 0 ? c : CUDART_INF_F;
                         if (halo) { /* neighbour across the cut of a winner next to it; nothing else changes */
-                            st[i].cp = st[i].k1 + dir == k ? c : st[i].cp;
+                            if (st[i].k1 + dir == k) nbr_at(i)->y = c;
                         } else {
                             n_eval += ci;
-                            st[i].template update<!SPLIT>(c, k, dir, desc, it == 0);
+                            st[i].template update<false>(c, k, dir, desc, it == 0, nbr_at(i));
                         }
                     }
                     if (dbg) {
@@ -866,6 +873,11 @@ __global__ void __launch_bounds__(Geo<WIN>::NT, 1) sweep_kernel(const __grid_con
          * the other one merges it into its registers and goes on.  State per pixel: b1, k1, s2, cm, cp and m2 = the
          * lowest cost of the half's planes except the one next to the cut (visited last). ----------------------- */
         bool do_epilogue = true;
+#pragma unroll
+        for (int i = 0; i < RPT; ++i) {
+            const float2 n = *nbr_at(i);
+            st[i].cm = n.x; st[i].cp = n.y;
+        }
         if (desc) {
 #pragma unroll
             for (int i = 0; i < RPT; ++i) st[i].swap_neighbours();
@@ -1004,38 +1016,40 @@ __global__ void __launch_bounds__(Geo<WIN>::NT, 1) sweep_kernel(const __grid_con
 }
 
 /* Kernel variants (fsw_api.cu: pick_variant): projection mode 0..2 (see SweepInst::go) + 3 if the footprints are
- * 8-byte bfloat16, + 6 for the plane split (two work items per tile). */
+ * 8-byte bfloat16; 6, 7 = modes 1, 2 with bfloat16 footprints for views whose image circle lies inside the raster (no
+ * border test); + 8 for the plane split (two work items per tile). */
 template <int WIN, int NVT>
 struct SweepInst {
     using G = Geo<WIN>;
     static constexpr bool FUSE = G::FUSE_OK && NVT != 1;
     /* MODE 0: any rotation, full distortion polynomial, denominator test; 1: identity rotations, k1-only distortion;
      * 2: any rotation, k1-only distortion (the last two need cos(fov/2) + xi >= 1e-3) */
-    template <int MODE, bool F16, bool SPLIT>
+    template <int MODE, bool F16, bool INSIDE, bool SPLIT>
     static cudaError_t go(const FswSweepArgs& args, int grid, cudaStream_t stream, bool prepare_only) {
-        auto kern = sweep_kernel<WIN, NVT, MODE == 1, MODE == 0, MODE == 0, F16, SPLIT>;
+        auto kern = sweep_kernel<WIN, NVT, MODE == 1, MODE == 0, MODE == 0, INSIDE, F16, SPLIT>;
         if (prepare_only) return cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::smem(FUSE));
         kern<<<grid, G::NT, G::smem(FUSE), stream>>>(args);
         return cudaGetLastError();
     }
-    static constexpr int N_VARIANTS = 12;
-    static cudaError_t dispatch(const FswSweepArgs& args, int variant, int grid, cudaStream_t stream, bool prep) {
+    static constexpr int N_VARIANTS = 16;
+    template <bool SPLIT>
+    static cudaError_t dispatch8(const FswSweepArgs& args, int variant, int grid, cudaStream_t stream, bool prep) {
         switch (variant) {
-            case 0: return go<0, false, false>(args, grid, stream, prep);
-            case 1: return go<1, false, false>(args, grid, stream, prep);
-            case 2: return go<2, false, false>(args, grid, stream, prep);
-            case 3: return go<0, true, false>(args, grid, stream, prep);
-            case 4: return go<1, true, false>(args, grid, stream, prep);
-            case 5: return go<2, true, false>(args, grid, stream, prep);
-            case 6: return go<0, false, true>(args, grid, stream, prep);
-            case 7: return go<1, false, true>(args, grid, stream, prep);
-            case 8: return go<2, false, true>(args, grid, stream, prep);
-            case 9: return go<0, true, true>(args, grid, stream, prep);
-            case 10: return go<1, true, true>(args, grid, stream, prep);
-            case 11: return go<2, true, true>(args, grid, stream, prep);
+            case 0: return go<0, false, false, SPLIT>(args, grid, stream, prep);
+            case 1: return go<1, false, false, SPLIT>(args, grid, stream, prep);
+            case 2: return go<2, false, false, SPLIT>(args, grid, stream, prep);
+            case 3: return go<0, true, false, SPLIT>(args, grid, stream, prep);
+            case 4: return go<1, true, false, SPLIT>(args, grid, stream, prep);
+            case 5: return go<2, true, false, SPLIT>(args, grid, stream, prep);
+            case 6: return go<1, true, true, SPLIT>(args, grid, stream, prep);
+            case 7: return go<2, true, true, SPLIT>(args, grid, stream, prep);
             default: break;
         }
         return cudaErrorInvalidValue;
+    }
+    static cudaError_t dispatch(const FswSweepArgs& args, int variant, int grid, cudaStream_t stream, bool prep) {
+        return variant < 8 ? dispatch8<false>(args, variant, grid, stream, prep)
+                           : dispatch8<true>(args, variant - 8, grid, stream, prep);
     }
     static cudaError_t launch(const FswSweepArgs& args, int variant, int grid, cudaStream_t stream) {
         return dispatch(args, variant, grid, stream, false);
