@@ -41,7 +41,7 @@ extern "C" {
 #endif
 
 #define FSW_VERSION_MAJOR 0
-#define FSW_VERSION_MINOR 2
+#define FSW_VERSION_MINOR 3
 
 /* status codes */
 #define FSW_OK 0
@@ -136,6 +136,17 @@ typedef struct fsw_sweep_params {
     float var_floor; /* floor of sqrt(var_a var_b) in the ZNCC denominator, in intensity units squared */
     float range_max; /* a ray/plane intersection further than this (metres along the ray) is invalid */
     float* debug_cost_volume; /* device, nullable: [P][H][W] float32, view-averaged cost, +inf = undefined */
+    /* Variants (readings Q26, Q27); 0 = the default behaviour described above.
+     * best_k: occlusion-robust view aggregation: the cost of a plane is the mean of the best_k lowest
+     *   per-view costs among the valid views (of all valid ones if fewer than best_k are valid) instead of the mean
+     *   over all valid views.  Supported: 0 (off), 1, 2; other values give FSW_E_UNSUPPORTED.
+     * filter_before_merge (read from params_crop by the multi-resolution calls): each scale is filtered on its own
+     *   -- the half-resolution pass with the thresholds of params_low, whose horizon_row counts half-resolution rows
+     *   -- and inside the crop the full-resolution estimate wins where it SURVIVED its filters, else a surviving
+     *   upsampled estimate fills in; an invalid pixel reports the reason of the estimate the default order would have
+     *   taken. */
+    int32_t best_k;
+    int32_t filter_before_merge;
 } fsw_sweep_params;
 
 /* one input image: row-major, pitch in BYTES */

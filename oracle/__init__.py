@@ -45,7 +45,7 @@ class Params(ctypes.Structure):
                 ("roi_x0", ctypes.c_int32), ("roi_y0", ctypes.c_int32), ("roi_w", ctypes.c_int32), ("roi_h", ctypes.c_int32),
                 ("horizon_row", ctypes.c_int32),
                 ("alpha_upper", ctypes.c_double), ("alpha_lower", ctypes.c_double), ("beta", ctypes.c_double),
-                ("var_floor", ctypes.c_double), ("range_max", ctypes.c_double)]
+                ("var_floor", ctypes.c_double), ("range_max", ctypes.c_double), ("best_k", ctypes.c_int32)]
 
 
 def build(force: bool = False) -> str:
@@ -157,6 +157,7 @@ def make_params(p) -> Params:
     out.alpha_upper, out.alpha_lower = float(p.get("alpha_upper", 1.0)), float(p.get("alpha_lower", 1.0))
     out.beta, out.var_floor = float(p.get("beta", 1.0)), float(p["var_floor"])
     out.range_max = float(p["range_max"])
+    out.best_k = int(p.get("best_k", 0))
     return out
 
 
@@ -333,7 +334,11 @@ def compute_depth(cams, ref_index, fams, params, images, mask=None, keep_cost=Fa
 
 def compute_depth_multires(cams, ref_index, fams_low, fams_crop, params_low, params_crop, crop, images, mask=None,
                            keep_cost=False):
-    """S10: half-resolution full-FOV pass + full-resolution crop pass, merged, then filters (params_crop) and mask."""
+    """S10: half-resolution full-FOV pass + full-resolution crop pass, merged, then filters (params_crop) and mask
+    (reading Q20).  With params_crop['filter_before_merge'] the other order of Q20 (reading Q27): each pass is filtered
+    on its own (the half-resolution one with params_low, whose horizon_row counts half-resolution rows), then inside
+    the crop the full-resolution estimate wins where it SURVIVED its filters, else the surviving upsampled one; then
+    the mask."""
     cams_c = [make_camera(c) for c in cams]
     cams_lo = [camera_half(c) for c in cams_c]
     imgs_lo = [downsample2(im) for im in images]
@@ -344,9 +349,37 @@ def compute_depth_multires(cams, ref_index, fams_low, fams_crop, params_low, par
     cost_hi, n_hi, frag_hi = sweep(cams_c, ref_index, fams_crop, p_hi, images)
     hi = wta(cams_c[ref_index], fams_crop, p_hi, cost_hi)
     H, W = cams_c[ref_index].height, cams_c[ref_index].width
-    maps = merge(W, H, crop, lo, hi)
-    filter_mask(params_crop, maps, mask)
-    frag = np.repeat(np.repeat(frag_lo, 2, axis=0), 2, axis=1)[:H, :W] | frag_hi
+    up = lambda a: np.repeat(np.repeat(a, 2, axis=0), 2, axis=1)[:H, :W]
+    if params_crop.get("filter_before_merge"):
+        filter_mask(params_low, lo)
+        filter_mask(p_hi, hi)
+        x0, y0, cw, ch = [int(v) for v in crop]
+        in_crop = np.zeros((H, W), dtype=bool)
+        in_crop[y0:y0 + ch, x0:x0 + cw] = True
+        pad = lambda a, fill: np.pad(up(a), ((0, H - up(a).shape[0]), (0, W - up(a).shape[1])), constant_values=fill)
+        lo_valid, lo_raw = pad(lo["valid"], 0) != 0, pad(lo["raw_valid"], 0) != 0
+        hi_valid, hi_raw = in_crop & (hi["valid"] != 0), in_crop & (hi["raw_valid"] != 0)
+        # where the values come from: a surviving estimate first (full resolution before half resolution), else the
+        # estimate the other order would have taken (it says why the pixel is invalid)
+        from_hi = hi_valid | (~lo_valid & hi_raw)
+        from_lo = ~from_hi & lo_raw
+        maps = {}
+        for key, fill in (("depth", 0.0), ("c1", np.inf), ("c2", np.inf)):
+            maps[key] = np.where(from_hi, hi[key], np.where(from_lo, pad(lo[key], fill), fill))
+        maps["kbest"] = np.where(from_hi, hi["kbest"] | (1 << 14), np.where(from_lo, pad(lo["kbest"], -1), -1)).astype(np.int32)
+        maps["raw_valid"] = (from_hi | from_lo).astype(np.uint8)
+        reason = np.where(from_hi, hi["reason"], np.where(from_lo, pad(lo["reason"], NO_PLANE), NO_PLANE)).astype(np.uint8)
+        if mask is not None:
+            masked = (reason == OK) & (np.asarray(mask) != 0)
+            reason[masked] = MASKED
+        maps["depth"] = np.where(reason == OK, maps["depth"], 0.0)
+        maps["reason"], maps["valid"] = reason, (reason == OK).astype(np.uint8)
+        maps["fragile_thr"] = (pad(lo["fragile_thr"], 0) | hi["fragile_thr"]).astype(np.uint8)
+    else:
+        maps = merge(W, H, crop, lo, hi)
+        filter_mask(params_crop, maps, mask)
+    frag = up(frag_lo)
+    frag = np.pad(frag, ((0, H - frag.shape[0]), (0, W - frag.shape[1]))) | frag_hi
     maps.update(n_eval=n_lo + n_hi, fragile_geom=frag, lo=lo, hi=hi)
     if keep_cost:
         maps["cost_lo"], maps["cost_hi"] = cost_lo, cost_hi

@@ -299,17 +299,20 @@ int orc_sweep(const orc_camera* cams, int n_cams, int ref_index, const orc_famil
 
     double* B = (double*)malloc(sizeof(double) * npx);    /* plane-warped view image, NaN = NONE */
     uint8_t* Bnear = (uint8_t*)malloc(npx);
-    double* acc = (double*)malloc(sizeof(double) * npx);
-    int32_t* cnt = (int32_t*)malloc(sizeof(int32_t) * npx);
+    /* per-view costs of the current plane, +inf where the view is invalid: [view slot][pixel] */
+    int n_views = n_cams - 1;
+    double* vcost = (double*)malloc(sizeof(double) * npx * (size_t)n_views);
     if (fragile_geom) memset(fragile_geom, 0, npx);
     int64_t evals = 0;
 
     for (int k = 0; k < P; ++k) {
         const double* n = nrm + 3 * pf[k];
-        memset(acc, 0, sizeof(double) * npx);
-        memset(cnt, 0, sizeof(int32_t) * npx);
+        for (size_t i = 0; i < npx * (size_t)n_views; ++i) vcost[i] = INFINITY;
+        int slot = -1;
         for (int v = 0; v < n_cams; ++v) {
             if (v == ref_index) continue;
+            ++slot;
+            double* vc = vcost + (size_t)slot * npx;
             const orc_camera* view = &cams[v];
             double R[9], T[3];
             orc_relative_pose(ref, view, R, T);
@@ -344,18 +347,37 @@ int orc_sweep(const orc_camera* cams, int n_cams, int ref_index, const orc_famil
                         }
                     if (near && fragile_geom) fragile_geom[i] = 1;
                     if (!ok) continue; /* view invalid for this (p,k) */
-                    acc[i] += orc_zncc_cost(wa, wb, N, prm->var_floor);
-                    cnt[i] += 1;
+                    vc[i] = orc_zncc_cost(wa, wb, N, prm->var_floor);
                     evals += 1;
                 }
             }
         }
-        /* O6: mean over valid views, +inf if none */
+        /* O6: mean over the valid views in fixed view order (Q11), +inf if none; with best_k > 0 the mean of the
+         * best_k lowest valid per-view costs instead (Q26), summed in ascending order of cost */
         double* ck = cost + (size_t)k * npx;
-        for (size_t i = 0; i < npx; ++i) ck[i] = cnt[i] > 0 ? acc[i] / (double)cnt[i] : INFINITY;
+        for (size_t i = 0; i < npx; ++i) {
+            double c[64];
+            int m = 0;
+            for (int sl = 0; sl < n_views; ++sl)
+                if (isfinite(vcost[(size_t)sl * npx + i])) c[m++] = vcost[(size_t)sl * npx + i];
+            if (m == 0) { ck[i] = INFINITY; continue; }
+            int use = m;
+            if (prm->best_k > 0 && prm->best_k < m) {
+                for (int a = 1; a < m; ++a) { /* insertion sort, ascending */
+                    double t = c[a];
+                    int b = a - 1;
+                    while (b >= 0 && c[b] > t) { c[b + 1] = c[b]; --b; }
+                    c[b + 1] = t;
+                }
+                use = prm->best_k;
+            }
+            double sum = 0.0;
+            for (int a = 0; a < use; ++a) sum += c[a];
+            ck[i] = sum / (double)use;
+        }
     }
     if (n_eval) *n_eval = evals;
-    free(pd); free(pf); free(nrm); free(ray); free(ray_ok); free(ray_near); free(B); free(Bnear); free(acc); free(cnt);
+    free(pd); free(pf); free(nrm); free(ray); free(ray_ok); free(ray_near); free(B); free(Bnear); free(vcost);
     return P;
 }
 
@@ -370,7 +392,7 @@ int orc_pixel_costs(const orc_camera* cams, int n_cams, int ref_index, const orc
     double* nrm = (double*)malloc(sizeof(double) * 3 * n_fams);
     orc_plane_table(fams, n_fams, 0, pd, pf, nrm);
     for (int k = 0; k < P; ++k) {
-        double sum = 0.0; int cnt = 0;
+        double cv[64]; int cnt = 0;
         for (int v = 0; v < n_cams; ++v) {
             if (v == ref_index) continue;
             double wa[31 * 31], wb[31 * 31];
@@ -386,10 +408,21 @@ int orc_pixel_costs(const orc_camera* cams, int n_cams, int ref_index, const orc
                     ++m;
                 }
             if (!ok) continue;
-            sum += orc_zncc_cost(wa, wb, N, prm->var_floor);
-            ++cnt;
+            cv[cnt++] = orc_zncc_cost(wa, wb, N, prm->var_floor);
         }
-        cost_out[k] = cnt ? sum / cnt : INFINITY;
+        int use = cnt;
+        if (prm->best_k > 0 && prm->best_k < cnt) {
+            for (int a = 1; a < cnt; ++a) {
+                double t = cv[a];
+                int b = a - 1;
+                while (b >= 0 && cv[b] > t) { cv[b + 1] = cv[b]; --b; }
+                cv[b + 1] = t;
+            }
+            use = prm->best_k;
+        }
+        double sum = 0.0;
+        for (int a = 0; a < use; ++a) sum += cv[a];
+        cost_out[k] = cnt ? sum / use : INFINITY;
     }
     free(pd); free(pf); free(nrm);
     return P;

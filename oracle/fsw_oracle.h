@@ -71,6 +71,9 @@ typedef struct {
     double beta;                     /* keep iff c2 >= beta*max(c1,1e-6) */
     double var_floor;                /* eps_v: floor of sqrt(var_a var_b) */
     double range_max;                /* NONE if the ray/plane range exceeds this */
+    int32_t best_k;                  /* view aggregation (reading Q26; "occlusion-robust best-k"): 0 = mean
+                                        over all valid views (Q11); k > 0 = mean of the k lowest per-view costs among
+                                        the valid views (all of them if fewer than k are valid) */
 } orc_params;
 
 /* O1: unified projective model.  Return 1 = valid, 0 = NONE. */

@@ -61,7 +61,7 @@ class CParams(ctypes.Structure):
                 ("filters_enabled", ctypes.c_int32), ("depth_kind", ctypes.c_int32), ("roi", CRect),
                 ("horizon_row", ctypes.c_int32), ("alpha_upper", ctypes.c_float), ("alpha_lower", ctypes.c_float),
                 ("beta", ctypes.c_float), ("var_floor", ctypes.c_float), ("range_max", ctypes.c_float),
-                ("debug_cost_volume", ctypes.c_void_p)]
+                ("debug_cost_volume", ctypes.c_void_p), ("best_k", ctypes.c_int32), ("filter_before_merge", ctypes.c_int32)]
 
 
 class CImage(ctypes.Structure):
@@ -184,6 +184,7 @@ def make_params(p, debug_cost_ptr=None) -> CParams:
     out.alpha_upper, out.alpha_lower = float(p.get("alpha_upper", 1.0)), float(p.get("alpha_lower", 1.0))
     out.beta, out.var_floor, out.range_max = float(p.get("beta", 1.0)), float(p["var_floor"]), float(p["range_max"])
     out.debug_cost_volume = debug_cost_ptr
+    out.best_k, out.filter_before_merge = int(p.get("best_k", 0)), int(p.get("filter_before_merge", 0))
     return out
 
 

@@ -112,7 +112,7 @@ struct fsw_context {
     std::vector<DevBuf> foot;      /* footprint images of the views: [set slot][camera] */
     std::vector<DevBuf> half;      /* half-resolution float images: [set slot][camera] */
     std::vector<DevBuf> half_foot; /* ... and their footprint images */
-    std::vector<DevBuf> lo_depth, lo_c1, lo_c2, lo_k; /* raw maps of the half-resolution pass: [set slot] */
+    std::vector<DevBuf> lo_depth, lo_c1, lo_c2, lo_k, lo_reason; /* maps of the half-resolution pass: [set slot] */
     DevBuf ctrl;                   /* FSW_CTRL_WORDS x uint32 */
     DevBuf sets_dev, sets_dev2;    /* FswSetPtrs of a batch (second table: the crop pass of a multi-resolution batch) */
     /* host side of the set table: a ring of pinned buffers, each guarded by an event recorded after its upload, so
@@ -241,6 +241,8 @@ int32_t check_params(const fsw_sweep_params* p, const char* name) {
     if (!(p->range_max > 0.f)) return fail(FSW_E_INVALID_ARG, "%s: range_max must be positive", name);
     if (!(p->var_floor >= 0.f)) return fail(FSW_E_INVALID_ARG, "%s: var_floor must be >= 0", name);
     if (!std::isfinite(p->alpha_upper) || !std::isfinite(p->alpha_lower) || !std::isfinite(p->beta)) return fail(FSW_E_INVALID_ARG, "%s: thresholds must be finite", name);
+    if (p->best_k < 0) return fail(FSW_E_INVALID_ARG, "%s: best_k=%d must be >= 0", name, p->best_k);
+    if (p->best_k > 2) return fail(FSW_E_UNSUPPORTED, "%s: best_k=%d: the kernels aggregate the best one or two views (or all)", name, p->best_k);
     return FSW_OK;
 }
 
@@ -327,6 +329,7 @@ int32_t fill_args(FswSweepArgs& a, const fsw_rig& rig, const fsw_planeset& ps, c
     a.floor2 = (float)(fl * fl);
     if (!(a.floor2 > 0.f)) a.floor2 = 1e-30f; /* keeps the reciprocal square root finite on flat windows */
     a.inv_range_max = 1.f / p.range_max;
+    a.best_k = p.best_k < a.n_views ? p.best_k : 0; /* the best k of k views or fewer is the plain mean */
     for (int c = 0; c < FSW_MAX_CAMERAS; ++c) a.inv_count[c] = c > 0 ? 1.f / (float)c : 0.f;
     a.n_sets = 1;
     return FSW_OK;
@@ -793,7 +796,7 @@ int32_t fsw_context_destroy(fsw_context* ctx) {
     if (!ctx) return FSW_OK;
     DeviceGuard g;
     g.enter(ctx->device);
-    for (std::vector<DevBuf>* v : {&ctx->foot, &ctx->half, &ctx->half_foot, &ctx->lo_depth, &ctx->lo_c1, &ctx->lo_c2, &ctx->lo_k,
+    for (std::vector<DevBuf>* v : {&ctx->foot, &ctx->half, &ctx->half_foot, &ctx->lo_depth, &ctx->lo_c1, &ctx->lo_c2, &ctx->lo_k, &ctx->lo_reason,
                                    &ctx->st_img, &ctx->st_mask, &ctx->st_depth, &ctx->st_c1, &ctx->st_c2, &ctx->st_k, &ctx->st_reason})
         for (DevBuf& b : *v) b.release();
     ctx->ctrl.release(); ctx->sets_dev.release(); ctx->sets_dev2.release();
@@ -906,8 +909,9 @@ static int32_t run_multires(fsw_context* ctx, const fsw_planeset* planes_low, co
     ctx->last_split = 0;
     const size_t ns = (size_t)n_sets;
     if (ctx->half.size() < ns * FSW_MAX_CAMERAS) ctx->half.resize(ns * FSW_MAX_CAMERAS);
-    for (std::vector<DevBuf>* v : {&ctx->lo_depth, &ctx->lo_c1, &ctx->lo_c2, &ctx->lo_k})
+    for (std::vector<DevBuf>* v : {&ctx->lo_depth, &ctx->lo_c1, &ctx->lo_c2, &ctx->lo_k, &ctx->lo_reason})
         if (v->size() < ns) v->resize(ns);
+    const bool filter_first = params_crop->filter_before_merge != 0;
 
     /* S10(a): 2x2 box downsample of every image of every set */
     FswDownArgs dn;
@@ -931,7 +935,9 @@ static int32_t run_multires(fsw_context* ctx, const fsw_planeset* planes_low, co
     const int LW = ref.width / 2, LH = ref.height / 2;
     FswSweepArgs a;
     fsw_sweep_params pl = *params_low;
-    pl.filters_enabled = 0; /* filters run after the merge (reading Q20) */
+    /* filters run after the merge (reading Q20), unless the caller asks for the other order (Q27): then the
+     * half-resolution pass applies its own and hands its verdicts to the crop pass */
+    if (!filter_first) pl.filters_enabled = 0;
     fill_args(a, rig, *planes_low, pl, true);
     std::vector<FswSetPtrs> sets(ns);
     std::memset(sets.data(), 0, sizeof(FswSetPtrs) * ns);
@@ -946,6 +952,10 @@ static int32_t run_multires(fsw_context* ctx, const fsw_planeset* planes_low, co
         lo.out_c1 = (float*)ctx->lo_c1[s].p; lo.out_c1_pitch = (int64_t)LW * 4;
         lo.out_c2 = (float*)ctx->lo_c2[s].p; lo.out_c2_pitch = (int64_t)LW * 4;
         lo.out_k = (int16_t*)ctx->lo_k[s].p; lo.out_k_pitch = (int64_t)LW * 2;
+        if (filter_first) {
+            FSW_CUDA(ctx->lo_reason[s].reserve((size_t)LW * LH));
+            lo.out_reason = (uint8_t*)ctx->lo_reason[s].p; lo.out_reason_pitch = (int64_t)LW;
+        }
     }
     if ((rc = stage_views(ctx, nullptr, n_sets, true, sets.data(), stream, true, &a.foot_f16)) != FSW_OK) return rc;
     a.n_sets = n_sets;
@@ -972,6 +982,7 @@ static int32_t run_multires(fsw_context* ctx, const fsw_planeset* planes_low, co
         set_outputs(hi, &outs[s], masks ? masks[s] : nullptr, mask_pitch);
         hi.lo_depth = (const float*)ctx->lo_depth[s].p; hi.lo_c1 = (const float*)ctx->lo_c1[s].p;
         hi.lo_c2 = (const float*)ctx->lo_c2[s].p; hi.lo_k = (const int16_t*)ctx->lo_k[s].p;
+        hi.lo_reason = filter_first ? (const uint8_t*)ctx->lo_reason[s].p : nullptr;
     }
     if ((rc = stage_views(ctx, images, n_sets, false, sets.data(), stream, false, &a.foot_f16)) != FSW_OK) return rc;
     a.n_sets = n_sets;
@@ -982,6 +993,7 @@ static int32_t run_multires(fsw_context* ctx, const fsw_planeset* planes_low, co
         a.sets = (const FswSetPtrs*)ctx->sets_dev2.p;
     }
     a.lo_W = LW; a.lo_H = LH;
+    a.filter_first = filter_first ? 1 : 0;
     a.index_flag = FSW_INDEX_FROM_CROP;
     a.count_pixels = 1;
     if (ctx->timing) FSW_CUDA(cudaEventRecord(ctx->ev[0], stream));

@@ -69,6 +69,7 @@ struct FswSetPtrs {
     const float* lo_c1;
     const float* lo_c2;
     const int16_t* lo_k;
+    const uint8_t* lo_reason; /* filter-before-merge order: verdicts of the half-resolution pass, else null */
     /* S11 */
     const uint8_t* mask;
     int64_t mask_pitch;
@@ -100,6 +101,9 @@ struct FswSweepArgs {
                             (+inf when the bound does not apply): tiles entirely beyond it skip S1 */
     int32_t lo_W, lo_H;
     int32_t foot_f16;   /* 1: the footprint images hold four bfloat16 per pixel, 0: four floats */
+    int32_t best_k;       /* 0: mean over the valid views; 1, 2: mean of the lowest one / two per-view costs (run-time
+                             view loop only) */
+    int32_t filter_first; /* crop pass of a multi-resolution call in the filter-before-merge order */
     int32_t views_inside; /* 1: the field of view of every view lies inside its image (no border test needed) */
     int32_t index_flag; /* OR-ed into the plane index this pass writes (FSW_INDEX_FROM_CROP or 0) */
     /* frame sets: set0 inline for the single-set calls, `sets` (device array) for batches */

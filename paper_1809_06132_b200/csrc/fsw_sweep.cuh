@@ -724,6 +724,12 @@ __global__ void __launch_bounds__(Geo<WIN>::NT, 1) sweep_kernel(const __grid_con
                     unsigned cnt = 0; /* valid views per output, 4 bits each */
 #pragma unroll
                     for (int i = 0; i < RPT; ++i) acc[i] = 0.f;
+                    /* best-k view aggregation (reading Q26; run-time view loop only): the two lowest per-view costs */
+                    float bk1[NVT == 0 ? RPT : 1], bk2[NVT == 0 ? RPT : 1];
+                    if constexpr (NVT == 0) {
+#pragma unroll
+                        for (int i = 0; i < RPT; ++i) { bk1[i] = CUDART_INF_F; bk2[i] = CUDART_INF_F; }
+                    }
                     /* S2: the plane is out of reach for the whole tile if even the best-facing ray is beyond range */
                     if (qmax * inv_d >= args.inv_range_max) {
                         const bool rows_on = qmax_w * inv_d >= args.inv_range_max; /* any ray of this warp's rows */
@@ -815,6 +821,12 @@ __global__ void __launch_bounds__(Geo<WIN>::NT, 1) sweep_kernel(const __grid_con
                                     float cst = __saturatef(fmaf(-0.5f, z, 0.5f));
                                     acc[i] += okv ? cst : 0.f;
                                     cnt += okv ? (1u << (4 * i)) : 0u;
+                                    if constexpr (NVT == 0) {
+                                        const float cv = okv ? cst : CUDART_INF_F;
+                                        const float hi = fmaxf(bk1[i], cv);
+                                        bk1[i] = fminf(bk1[i], cv);
+                                        bk2[i] = fminf(bk2[i], hi);
+                                    }
                                 }
                             }
                         };
@@ -841,6 +853,10 @@ __global__ void __launch_bounds__(Geo<WIN>::NT, 1) sweep_kernel(const __grid_con
                         if (NVT == 1) c = acc[i];
                         else if (NVT == 2) c = ci == 2 ? 0.5f * acc[i] : acc[i];
                         else c = ci == n_views ? acc[i] * inv_views : acc[i] * args.inv_count[ci];
+                        if constexpr (NVT == 0) {
+                            if (args.best_k == 1) c = bk1[i];
+                            else if (args.best_k == 2) c = ci >= 2 ? 0.5f * (bk1[i] + bk2[i]) : bk1[i];
+                        }
                         c = ci > 0 ? c : CUDART_INF_F;
                         if (halo) { /* neighbour across the cut of a winner next to it; nothing else changes */
                             if (st[i].k1 + dir == k) nbr_at(i)->y = c;
@@ -962,26 +978,47 @@ __global__ void __launch_bounds__(Geo<WIN>::NT, 1) sweep_kernel(const __grid_con
                 c1 = st[i].b1;
                 c2 = st[i].s2 < CUDART_INF_F ? st[i].s2 : 1.f;
                 kidx = st[i].k1 | args.index_flag;
-            } else if (S.lo_k != nullptr) {
-                /* S10(c)-(e): nearest-neighbour upsample of the half-resolution pass */
-                int xl = ox >> 1, yl = oy >> 1;
-                if (xl < args.lo_W && yl < args.lo_H) {
-                    int64_t j = (int64_t)yl * args.lo_W + xl;
-                    int kl = S.lo_k[j];
-                    if (kl >= 0) {
+            }
+            /* S9: verdict of the cost / ratio filters on a (best, second best) pair of this row */
+            auto verdict = [&](const float b, const float sec) -> int {
+                const float alpha = oy < args.horizon_row ? args.alpha_upper : args.alpha_lower;
+                if ((args.filters & FSW_FILTER_COST) && b > alpha) return FSW_REASON_COST_FILTER;
+                if ((args.filters & FSW_FILTER_RATIO) && sec < args.beta * fmaxf(b, 1e-6f)) return FSW_REASON_RATIO_FILTER;
+                return FSW_REASON_OK;
+            };
+            int reason;
+            if (S.lo_k != nullptr) {
+                /* S10(c)-(e): merge with the nearest-neighbour upsampled half-resolution pass */
+                const int xl = ox >> 1, yl = oy >> 1;
+                const bool lo_in = xl < args.lo_W && yl < args.lo_H;
+                const int64_t j = lo_in ? (int64_t)yl * args.lo_W + xl : 0;
+                const int kl = lo_in ? (int)S.lo_k[j] : -1;
+                if (!args.filter_first) {
+                    /* reading Q19 / Q20: full resolution where it has any finite plane, else the upsampled estimate;
+                     * the filters see the merged map */
+                    if (!raw_valid && kl >= 0) {
                         raw_valid = true;
                         depth = S.lo_depth[j]; c1 = S.lo_c1[j]; c2 = S.lo_c2[j]; kidx = kl;
                     }
+                    reason = raw_valid ? verdict(c1, c2) : FSW_REASON_NO_PLANE;
+                } else {
+                    /* reading Q27: each scale filtered on its own; a surviving full-resolution estimate wins, else a
+                     * surviving upsampled one fills in; otherwise the pixel reports the estimate (and the reason) the
+                     * default order would have taken */
+                    reason = raw_valid ? verdict(c1, c2) : FSW_REASON_NO_PLANE;
+                    if (reason != FSW_REASON_OK && kl >= 0) {
+                        const int lo_reason = S.lo_reason[j];
+                        if (lo_reason == FSW_REASON_OK || !raw_valid) {
+                            raw_valid = true;
+                            depth = S.lo_depth[j]; c1 = S.lo_c1[j]; c2 = S.lo_c2[j]; kidx = kl;
+                            reason = lo_reason;
+                        }
+                    }
                 }
+            } else {
+                reason = raw_valid ? verdict(c1, c2) : FSW_REASON_NO_PLANE;
             }
-            int reason = FSW_REASON_OK;
-            if (!raw_valid) reason = FSW_REASON_NO_PLANE;
-            else {
-                float alpha = oy < args.horizon_row ? args.alpha_upper : args.alpha_lower;
-                if ((args.filters & FSW_FILTER_COST) && c1 > alpha) reason = FSW_REASON_COST_FILTER;
-                else if ((args.filters & FSW_FILTER_RATIO) && c2 < args.beta * fmaxf(c1, 1e-6f)) reason = FSW_REASON_RATIO_FILTER;
-                else if (S.mask != nullptr && S.mask[(int64_t)oy * S.mask_pitch + ox]) reason = FSW_REASON_MASKED;
-            }
+            if (reason == FSW_REASON_OK && S.mask != nullptr && S.mask[(int64_t)oy * S.mask_pitch + ox]) reason = FSW_REASON_MASKED;
             if (reason != FSW_REASON_OK) depth = 0.f;
             n_raw += raw_valid ? 1u : 0u;
             n_ok += reason == FSW_REASON_OK ? 1u : 0u;
@@ -1066,9 +1103,11 @@ struct SweepInst {
 
 /* Which instantiation serves a call: up to four views (the paper's rig has four matching views) have
  * their view loop unrolled, pairs of views sharing a pass; more views, or three / four views with the large windows
- * that cannot pair them, take the run-time loop (NVT = 0). */
+ * that cannot pair them, take the run-time loop (NVT = 0); so do calls with best-k view aggregation (its two extra
+ * registers per output stay out of the kernels that serve the default). */
 template <int WIN>
-constexpr int nvt_for(int n_views) {
+constexpr int nvt_for(int n_views, int best_k) {
+    if (best_k > 0) return 0;
     return n_views <= 2 ? n_views : ((n_views <= 4 && Geo<WIN>::FUSE_OK) ? n_views : 0);
 }
 

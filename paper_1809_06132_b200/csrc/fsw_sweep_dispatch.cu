@@ -16,14 +16,14 @@ FSW_DECL_LARGE(11) FSW_DECL_LARGE(13) FSW_DECL_LARGE(15)
     case n: return prep ? fsw_prepare_sweep_w##w##_v##n() : fsw_launch_sweep_w##w##_v##n(args, variant, grid, stream);
 #define FSW_WINDOW_SMALL(w)                                                                    \
     case w:                                                                                    \
-        switch (fsw::nvt_for<w>(n_views)) { FSW_CASE(w, 0) FSW_CASE(w, 1) FSW_CASE(w, 2) FSW_CASE(w, 3) FSW_CASE(w, 4) } \
+        switch (fsw::nvt_for<w>(n_views, best_k)) { FSW_CASE(w, 0) FSW_CASE(w, 1) FSW_CASE(w, 2) FSW_CASE(w, 3) FSW_CASE(w, 4) } \
         break;
 #define FSW_WINDOW_LARGE(w)                                                    \
     case w:                                                                    \
-        switch (fsw::nvt_for<w>(n_views)) { FSW_CASE(w, 0) FSW_CASE(w, 1) FSW_CASE(w, 2) } \
+        switch (fsw::nvt_for<w>(n_views, best_k)) { FSW_CASE(w, 0) FSW_CASE(w, 1) FSW_CASE(w, 2) } \
         break;
 
-static cudaError_t route(int window, int n_views, bool prep, const FswSweepArgs& args, int variant, int grid, cudaStream_t stream) {
+static cudaError_t route(int window, int n_views, int best_k, bool prep, const FswSweepArgs& args, int variant, int grid, cudaStream_t stream) {
     switch (window) {
         FSW_WINDOW_SMALL(3) FSW_WINDOW_SMALL(5) FSW_WINDOW_SMALL(7) FSW_WINDOW_SMALL(9)
         FSW_WINDOW_LARGE(11) FSW_WINDOW_LARGE(13) FSW_WINDOW_LARGE(15)
@@ -33,13 +33,15 @@ static cudaError_t route(int window, int n_views, bool prep, const FswSweepArgs&
 }
 
 cudaError_t fsw_launch_sweep(int window, const FswSweepArgs& args, int variant, int grid, cudaStream_t stream) {
-    return route(window, args.n_views, false, args, variant, grid, stream);
+    return route(window, args.n_views, args.best_k, false, args, variant, grid, stream);
 }
 
 /* sets the shared-memory attribute of every variant that can serve calls with this window and view count */
 cudaError_t fsw_prepare_sweep(int window, int n_views) {
     static const FswSweepArgs dummy = {};
-    return route(window, n_views, true, dummy, 0, 0, nullptr);
+    cudaError_t e = route(window, n_views, 0, true, dummy, 0, 0, nullptr);
+    if (e == cudaSuccess && n_views > 1) e = route(window, n_views, 1, true, dummy, 0, 0, nullptr); /* the best-k variant */
+    return e;
 }
 
 FswSweepGeometry fsw_sweep_geometry(int window, int n_views) {

@@ -33,7 +33,7 @@ def test_library_exports_every_declared_symbol():
     for name in names:
         assert hasattr(lib, name), name
     assert sorted(binding.EXPORTS) == names
-    assert fsw.version() == (0, 2)
+    assert fsw.version() == (0, 3)
 
 
 def test_struct_layouts_match_header():

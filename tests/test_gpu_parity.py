@@ -140,6 +140,78 @@ def test_multires_batch_host_small():
         ctx.compute_depth_multires_batch(pl, pc, p_lo, p_hi, (100, 27, 61, 40), sets, masks, host=True)   # crop leaves the image
 
 
+@pytest.mark.parametrize("n_views,best_k", [(2, 1), (4, 1), (4, 2), (3, 2), (2, 2)])
+def test_best_k_view_aggregation(n_views, best_k):
+    """SURVEY 8(f) 4 / reading Q26: the mean of the best_k lowest per-view costs.  One view is corrupted
+    in a band so that the aggregation rule matters; best_k >= views is the plain mean bit for bit."""
+    import torch
+    import paper_1809_06132_b200 as fsw
+    cfg = _small_rig(W=150, H=101, n_views=n_views, rot=True, fov=170.0)
+    images = synth.render_frame(dict(cfg, scene=synth.scene_boxes(seed=5)), 0)
+    images[1] = images[1].copy()
+    images[1][:, 40:90] = np.random.default_rng(3).integers(0, 255, (101, 50), dtype=np.uint8)
+    p = dict(cfg["params"], best_k=best_k, filters=3, alpha_upper=0.4, alpha_lower=0.4, beta=1.05, horizon_row=50)
+    fams = [synth.family((0, 0, 1), 24, 0.8, 30.0, "inverse"), synth.family((0, 1, 0), 5, 0.6, 1.6, "linear")]
+    _, _, ctx = gpu_objects(cfg)
+    ref, test, stats, _ = run_single(cfg, images, params=p, families=fams, ctx=ctx)
+    assert_gates(stats, depth_frac_over_tol=0.01)
+    plain, _, _, _ = run_single(cfg, images, params=dict(p, best_k=0), families=fams, ctx=ctx)
+    if best_k >= n_views:
+        assert np.array_equal(ref["kbest"], plain["kbest"])
+        planes = fsw.PlaneSet(fams)
+        dev = [torch.from_numpy(im).cuda() for im in images]
+        a = oracle.compare.to_numpy(ctx.compute_depth(planes, p, dev))
+        b = oracle.compare.to_numpy(ctx.compute_depth(planes, dict(p, best_k=0), dev))
+        for key in ("depth", "best_cost", "second_cost", "plane_index", "valid_reason"):
+            assert np.array_equal(a[key], b[key], equal_nan=True), key
+    else:
+        assert (ref["kbest"] != plain["kbest"]).sum() > 50      # the rule matters on this input
+        ctx.set_split("on")                                      # and the plane split carries it as well
+        _, split, stats2, _ = run_single(cfg, images, params=p, families=fams, ctx=ctx)
+        for key in ("depth", "best_cost", "second_cost", "plane_index", "valid_reason"):
+            assert np.array_equal(test[key], split[key], equal_nan=True), key
+    with pytest.raises(fsw.FswError) as ei:
+        ctx.compute_depth(fsw.PlaneSet(fams), dict(p, best_k=3), [torch.from_numpy(im).cuda() for im in images])
+    assert ei.value.code == fsw.binding.E_UNSUPPORTED
+
+
+def test_filter_before_merge_order():
+    """SURVEY 8(f) 4 / reading Q27: each scale filtered on its own, then merged -- against the oracle, with strict
+    thresholds for the crop pass so that half-resolution estimates fill in, single call and batch."""
+    import torch
+    import paper_1809_06132_b200 as fsw
+    cfg = _small_rig(W=128, H=96, n_views=2, fov=170.0)
+    images = synth.render_frame(dict(cfg, scene=synth.scene_boxes(seed=12, n_boxes=8)), 0)
+    cfg.update(families_low=[synth.family((0, 0, 1), 16, 0.8, 30.0, "inverse")],
+               families_crop=[synth.family((0, 0, 1), 32, 0.8, 40.0, "inverse")],
+               params_low=synth.params(5, synth.VAR_FLOOR_U8, 60.0, 0.25, 0.35, 24, 1.1, filters=3),
+               params_crop=dict(synth.params(7, synth.VAR_FLOOR_U8, 80.0, 0.03, 0.05, 48, 1.15, filters=3), filter_before_merge=1),
+               crop=(35, 27, 61, 40))
+    mask = np.zeros((96, 128), np.uint8)
+    mask[10:30, 50:90] = 1
+    _, _, ctx = gpu_objects(cfg)
+    ref, test, stats, _ = run_multires(cfg, images, mask, ctx=ctx)
+    assert_gates(stats, depth_frac_over_tol=0.01)
+    k = ref["kbest"]
+    x0, y0, w, h = cfg["crop"]
+    inside = np.zeros(mask.shape, bool)
+    inside[y0:y0 + h, x0:x0 + w] = True
+    filled = inside & (ref["reason"] == 0) & (k >= 0) & ((k >> 14) == 0)
+    assert filled.sum() > 20 and (inside & (ref["reason"] == 0) & ((k >> 14) == 1)).sum() > 20
+    other = dict(cfg, params_crop=dict(cfg["params_crop"], filter_before_merge=0))
+    ref2, _, stats2, _ = run_multires(other, images, mask, ctx=ctx)
+    assert_gates(stats2, depth_frac_over_tol=0.01)
+    assert (ref["reason"] == 0).sum() > (ref2["reason"] == 0).sum()      # filtering first keeps more
+    pl, pc = fsw.PlaneSet(cfg["families_low"]), fsw.PlaneSet(cfg["families_crop"])
+    dev = [torch.from_numpy(im).cuda() for im in images]
+    outs = ctx.compute_depth_multires_batch(pl, pc, cfg["params_low"], cfg["params_crop"], cfg["crop"], [dev, dev],
+                                            [torch.from_numpy(mask).cuda(), None])
+    torch.cuda.synchronize()
+    got = oracle.compare.to_numpy(outs[0])
+    for key in ("depth", "best_cost", "second_cost", "plane_index", "valid_reason"):
+        assert np.array_equal(test[key], got[key], equal_nan=True), key
+
+
 @pytest.mark.parametrize("idx", [1, 2])
 def test_config_with_filters(idx):
     """C1 / C2 name no filters; SURVEY 8(d) asks for both the raw-valid set and alpha = 0.3/0.3, beta = 1.2."""
