@@ -136,7 +136,7 @@ typedef struct fsw_sweep_params {
     float var_floor; /* floor of sqrt(var_a var_b) in the ZNCC denominator, in intensity units squared */
     float range_max; /* a ray/plane intersection further than this (metres along the ray) is invalid */
     float* debug_cost_volume; /* device, nullable: [P][H][W] float32, view-averaged cost, +inf = undefined */
-    /* Variants (readings Q26, Q27); 0 = the default behaviour described above.
+    /* Variants (readings Q26, Q27, Q28); 0 = the default behaviour described above.
      * best_k: occlusion-robust view aggregation: the cost of a plane is the mean of the best_k lowest
      *   per-view costs among the valid views (of all valid ones if fewer than best_k are valid) instead of the mean
      *   over all valid views.  Supported: 0 (off), 1, 2; other values give FSW_E_UNSUPPORTED.
@@ -144,9 +144,16 @@ typedef struct fsw_sweep_params {
      *   -- the half-resolution pass with the thresholds of params_low, whose horizon_row counts half-resolution rows
      *   -- and inside the crop the full-resolution estimate wins where it SURVIVED its filters, else a surviving
      *   upsampled estimate fills in; an invalid pixel reports the reason of the estimate the default order would have
-     *   taken. */
+     *   taken.
+     * upsample_plane (read from params_crop by the multi-resolution calls; the alternative of reading Q18): a
+     *   full-resolution pixel that takes the half-resolution estimate does not copy its range but intersects ITS OWN
+     *   ray with the refined plane the half-resolution pixel chose (depth = d* / (n.r), times r_z for FSW_DEPTH_Z);
+     *   where its ray lies outside the field of view or does not face that plane the pixel is invalid
+     *   (FSW_REASON_NO_PLANE).  Costs and index are copied. */
     int32_t best_k;
     int32_t filter_before_merge;
+    int32_t upsample_plane;
+    int32_t reserved_;
 } fsw_sweep_params;
 
 /* one input image: row-major, pitch in BYTES */

@@ -378,6 +378,30 @@ def compute_depth_multires(cams, ref_index, fams_low, fams_crop, params_low, par
     else:
         maps = merge(W, H, crop, lo, hi)
         filter_mask(params_crop, maps, mask)
+    if params_crop.get("upsample_plane"):
+        # alternative of reading Q18 (reading Q28): a pixel that takes the half-resolution estimate intersects ITS OWN
+        # ray with the refined plane the half-resolution pixel chose: range = d* / (n.r); outside the field of view or
+        # not facing the plane -> invalid (NO_PLANE).  Costs and index stay the copied ones.
+        s_lo, d_lo, f_lo, n_lo_fam = plane_table(fams_low)
+        depth_kind = int(params_crop.get("depth_kind", 0))
+        ys, xs = np.nonzero((maps["kbest"] >= 0) & ((maps["kbest"] >> 14) == 0))
+        for y, x in zip(ys, xs):
+            yl, xl = y >> 1, x >> 1
+            k = int(lo["kbest"][yl, xl])
+            sk = s_lo[k]
+            if lo["delta"][yl, xl] != 0.0:
+                sk = sk + lo["delta"][yl, xl] * (s_lo[k + 1] - s_lo[k])
+            f = int(f_lo[k])
+            d_star = 1.0 / sk if fams_low[f]["spacing"] in ("inverse", INVERSE) else sk
+            r = back_project(cams_c[ref_index], float(x), float(y))
+            q = -1.0 if r is None else float(n_lo_fam[f] @ r)
+            if q > 1e-9:
+                if maps["reason"][y, x] == OK:
+                    maps["depth"][y, x] = d_star / q * (r[2] if depth_kind == 1 else 1.0)
+            else:
+                maps["reason"][y, x] = NO_PLANE
+                maps["depth"][y, x] = 0.0
+        maps["valid"] = (maps["reason"] == OK).astype(np.uint8)
     frag = up(frag_lo)
     frag = np.pad(frag, ((0, H - frag.shape[0]), (0, W - frag.shape[1]))) | frag_hi
     maps.update(n_eval=n_lo + n_hi, fragile_geom=frag, lo=lo, hi=hi)

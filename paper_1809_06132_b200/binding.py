@@ -61,7 +61,8 @@ class CParams(ctypes.Structure):
                 ("filters_enabled", ctypes.c_int32), ("depth_kind", ctypes.c_int32), ("roi", CRect),
                 ("horizon_row", ctypes.c_int32), ("alpha_upper", ctypes.c_float), ("alpha_lower", ctypes.c_float),
                 ("beta", ctypes.c_float), ("var_floor", ctypes.c_float), ("range_max", ctypes.c_float),
-                ("debug_cost_volume", ctypes.c_void_p), ("best_k", ctypes.c_int32), ("filter_before_merge", ctypes.c_int32)]
+                ("debug_cost_volume", ctypes.c_void_p), ("best_k", ctypes.c_int32), ("filter_before_merge", ctypes.c_int32),
+                ("upsample_plane", ctypes.c_int32), ("reserved_", ctypes.c_int32)]
 
 
 class CImage(ctypes.Structure):
@@ -185,6 +186,7 @@ def make_params(p, debug_cost_ptr=None) -> CParams:
     out.beta, out.var_floor, out.range_max = float(p.get("beta", 1.0)), float(p["var_floor"]), float(p["range_max"])
     out.debug_cost_volume = debug_cost_ptr
     out.best_k, out.filter_before_merge = int(p.get("best_k", 0)), int(p.get("filter_before_merge", 0))
+    out.upsample_plane = int(p.get("upsample_plane", 0))
     return out
 
 

@@ -938,7 +938,9 @@ static int32_t run_multires(fsw_context* ctx, const fsw_planeset* planes_low, co
     /* filters run after the merge (reading Q20), unless the caller asks for the other order (Q27): then the
      * half-resolution pass applies its own and hands its verdicts to the crop pass */
     if (!filter_first) pl.filters_enabled = 0;
+    const bool up_plane = params_crop->upsample_plane != 0;
     fill_args(a, rig, *planes_low, pl, true);
+    if (up_plane) a.depth_kind = FSW_DEPTH_PLANE_OFFSET; /* the crop pass turns offsets into depths of its own rays */
     std::vector<FswSetPtrs> sets(ns);
     std::memset(sets.data(), 0, sizeof(FswSetPtrs) * ns);
     for (int s = 0; s < n_sets; ++s) {
@@ -994,6 +996,12 @@ static int32_t run_multires(fsw_context* ctx, const fsw_planeset* planes_low, co
     }
     a.lo_W = LW; a.lo_H = LH;
     a.filter_first = filter_first ? 1 : 0;
+    a.upsample_plane = up_plane ? 1 : 0;
+    a.n_lo_fams = planes_low->n_fams;
+    for (int f = 0; f < planes_low->n_fams; ++f) {
+        for (int i = 0; i < 3; ++i) a.lo_fam_n[f][i] = (float)planes_low->fams[f].normal[i];
+        a.lo_fam_first[f] = planes_low->first[f];
+    }
     a.index_flag = FSW_INDEX_FROM_CROP;
     a.count_pixels = 1;
     if (ctx->timing) FSW_CUDA(cudaEventRecord(ctx->ev[0], stream));

@@ -22,6 +22,9 @@
 #define FSW_DIST_K1 1   /* k1 only */
 #define FSW_DIST_FULL 2 /* k1,k2,p1,p2 */
 
+/* internal depth_kind of the half-resolution pass under plane-consistent upsampling: write the refined plane offset */
+#define FSW_DEPTH_PLANE_OFFSET 2
+
 /* Footprint image of a matching view (S4): four numbers per pixel (x,y),
  *   .x = I(x,y), .y = I(x+1,y) - I(x,y), .z = I(x,y+1), .w = I(x+1,y+1) - I(x,y+1)
  * so that one load fetches everything a bilinear sample needs:
@@ -104,6 +107,11 @@ struct FswSweepArgs {
     int32_t best_k;       /* 0: mean over the valid views; 1, 2: mean of the lowest one / two per-view costs (run-time
                              view loop only) */
     int32_t filter_first; /* crop pass of a multi-resolution call in the filter-before-merge order */
+    /* plane-consistent upsampling (crop pass): the half-resolution pass wrote plane offsets d* instead of ranges;
+     * normals and first plane index of ITS families */
+    int32_t upsample_plane, n_lo_fams;
+    float lo_fam_n[FSW_MAX_FAMILIES][3];
+    int32_t lo_fam_first[FSW_MAX_FAMILIES];
     int32_t views_inside; /* 1: the field of view of every view lies inside its image (no border test needed) */
     int32_t index_flag; /* OR-ed into the plane index this pass writes (FSW_INDEX_FROM_CROP or 0) */
     /* frame sets: set0 inline for the single-set calls, `sets` (device array) for batches */

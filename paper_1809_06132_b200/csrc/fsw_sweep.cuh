@@ -480,6 +480,25 @@ struct SetHot {
     float* debug_cost;
 };
 
+/* Plane-consistent upsampling (alternative of reading Q18, Q28): the value of a pixel came from the
+ * half-resolution pass as a plane offset d*; the pixel's own ray meets that plane at range d* / (n.r).  Out of line: a
+ * rarely used variant must not cost the sweep loop registers.  The ray is recomputed (tiles outside the crop never
+ * ran S1).  Returns the depth; sets reason = FSW_REASON_NO_PLANE where the ray does not meet the plane. */
+__device__ __noinline__ float plane_upsampled_depth(const FswSweepArgs& args, int ox, int oy, int kidx, float d_star, int& reason) {
+    int f = 0;
+    for (int g = 1; g < args.n_lo_fams; ++g)
+        if (kidx >= args.lo_fam_first[g]) f = g;
+    float rx = 0.f, ry = 0.f, rz = 0.f;
+    const bool in_fov = back_project(args.ref, (float)ox, (float)oy, rx, ry, rz);
+    const float q = fmaf(args.lo_fam_n[f][0], rx, fmaf(args.lo_fam_n[f][1], ry, args.lo_fam_n[f][2] * rz));
+    if (in_fov && q > FSW_EPS_Q) {
+        const float range = d_star / q;
+        return args.depth_kind == FSW_DEPTH_Z ? range * rz : range;
+    }
+    reason = FSW_REASON_NO_PLANE;
+    return d_star;
+}
+
 /* NVT = number of views known at compile time (1..4), 0 = read args.n_views at run time (then the view parameters
  * come from a copy in shared memory, not from dynamically indexed kernel parameters). */
 template <int WIN, int NVT, bool IDENT, bool FULLDIST, bool CHECKDEN, bool INSIDE, bool F16, bool SPLIT>
@@ -974,7 +993,7 @@ __global__ void __launch_bounds__(Geo<WIN>::NT, 1) sweep_kernel(const __grid_con
                 float4 ry = rays[(grp * RPT + i + HW) * G::SB + col + HW];
                 float q = fmaf(F.n[0], ry.x, fmaf(F.n[1], ry.y, F.n[2] * ry.z));
                 float range = d / q;
-                depth = args.depth_kind == FSW_DEPTH_Z ? range * ry.z : range;
+                depth = args.depth_kind == FSW_DEPTH_Z ? range * ry.z : (args.depth_kind == FSW_DEPTH_PLANE_OFFSET ? d : range);
                 c1 = st[i].b1;
                 c2 = st[i].s2 < CUDART_INF_F ? st[i].s2 : 1.f;
                 kidx = st[i].k1 | args.index_flag;
@@ -1018,6 +1037,8 @@ __global__ void __launch_bounds__(Geo<WIN>::NT, 1) sweep_kernel(const __grid_con
             } else {
                 reason = raw_valid ? verdict(c1, c2) : FSW_REASON_NO_PLANE;
             }
+            if (args.upsample_plane && (kidx >= 0) && !(kidx & FSW_INDEX_FROM_CROP) && S.lo_k != nullptr)
+                depth = plane_upsampled_depth(args, ox, oy, kidx, depth, reason);
             if (reason == FSW_REASON_OK && S.mask != nullptr && S.mask[(int64_t)oy * S.mask_pitch + ox]) reason = FSW_REASON_MASKED;
             if (reason != FSW_REASON_OK) depth = 0.f;
             n_raw += raw_valid ? 1u : 0u;

@@ -212,6 +212,30 @@ def test_filter_before_merge_order():
         assert np.array_equal(test[key], got[key], equal_nan=True), key
 
 
+@pytest.mark.parametrize("depth_kind,filter_first", [(0, 0), (1, 1)])
+def test_plane_consistent_upsampling(depth_kind, filter_first):
+    """SURVEY 8(f) 4 / reading Q28: pixels that take the half-resolution estimate intersect their own ray with the
+    refined plane of the half-resolution pixel (range and z-depth, both merge orders), against the oracle."""
+    cfg = _small_rig(W=128, H=96, n_views=2, fov=170.0)
+    images = synth.render_frame(dict(cfg, scene=synth.scene_boxes(seed=12, n_boxes=8)), 0)
+    cfg.update(families_low=[synth.family((0, 0, 1), 16, 0.8, 30.0, "inverse"), synth.family((0, 1, 0), 4, 0.8, 1.6, "linear")],
+               families_crop=[synth.family((0, 0, 1), 32, 0.8, 40.0, "inverse")],
+               params_low=synth.params(5, synth.VAR_FLOOR_U8, 60.0, 0.3, 0.4, 24, 1.05, filters=3),
+               params_crop=dict(synth.params(7, synth.VAR_FLOOR_U8, 80.0, 0.2, 0.3, 48, 1.1, filters=3, depth_kind=depth_kind),
+                                upsample_plane=1, filter_before_merge=filter_first),
+               crop=(35, 27, 61, 40))
+    mask = np.zeros((96, 128), np.uint8)
+    mask[60:80, 20:60] = 1
+    ref, test, stats, _ = run_multires(cfg, images, mask)
+    assert_gates(stats, depth_frac_over_tol=0.01)
+    k = ref["kbest"]
+    from_lo = (k >= 0) & ((k >> 14) == 0) & (ref["reason"] == 0)
+    assert from_lo.sum() > 500
+    plain = dict(cfg, params_crop=dict(cfg["params_crop"], upsample_plane=0))
+    ref0, _, _, _ = run_multires(plain, images, mask)
+    assert (np.abs(ref0["depth"][from_lo] - ref["depth"][from_lo]) > 1e-6 * ref["depth"][from_lo]).mean() > 0.5
+
+
 @pytest.mark.parametrize("idx", [1, 2])
 def test_config_with_filters(idx):
     """C1 / C2 name no filters; SURVEY 8(d) asks for both the raw-valid set and alpha = 0.3/0.3, beta = 1.2."""

@@ -10,6 +10,11 @@ Reading Q27 -- filter each scale, then merge (the alternative order of Q20: SPEC
 paper's multi-scale experiment is unfiltered).  Pinned by its limiting cases: with thresholds that reject
 every full-resolution estimate the result is the filtered half-resolution map upsampled (fill-in), with thresholds
 that reject nothing both orders agree, and outside the crop the full-resolution pass never shows.
+
+Reading Q28 -- plane-consistent upsampling (the alternative SURVEY Q18 notes): a pixel that takes the half-resolution
+estimate intersects its own ray with the refined plane of the half-resolution pixel.  Pinned by geometry: the upsampled
+points of one half-resolution pixel lie ON that plane (n.X = d*), which the copied ranges do not; a fronto-parallel
+scene plane that coincides with a sweep plane comes back with the exact z at every upsampled pixel.
 """
 import numpy as np
 
@@ -140,3 +145,43 @@ def test_filter_before_merge_limiting_cases():
     for key in ("depth", "c1", "c2", "kbest", "reason"):
         assert np.array_equal(r1[key], r2[key]), key
     assert after["n_eval"] == first["n_eval"]
+
+
+def test_plane_consistent_upsampling_puts_the_points_on_the_chosen_plane():
+    cams, imgs, fl, fc, p_lo, p_hi, crop = _multires_setup()
+    H, W = imgs[0].shape
+    off = dict(filters=0)
+    copy = oracle.compute_depth_multires(cams, 0, fl, fc, dict(p_lo, **off), dict(p_hi, **off), crop, imgs)
+    plane = oracle.compute_depth_multires(cams, 0, fl, fc, dict(p_lo, **off), dict(p_hi, upsample_plane=1, **off), crop, imgs)
+    lo = plane["lo"]
+    s_lo, d_lo, f_lo, n_fam = oracle.plane_table(fl)
+    from_lo = (plane["kbest"] >= 0) & ((plane["kbest"] >> 14) == 0)
+    assert from_lo.sum() > 500
+    # costs, index and the pixels supplied by the crop pass are untouched
+    for key in ("c1", "c2", "kbest"):
+        assert np.array_equal(copy[key], plane[key]), key
+    hi_px = (plane["kbest"] >> 14) == 1
+    assert np.array_equal(copy["depth"][hi_px], plane["depth"][hi_px])
+    n_checked, off_plane_copy = 0, 0
+    for y, x in list(zip(*np.nonzero(from_lo & (plane["reason"] == 0))))[::7]:
+        yl, xl = y >> 1, x >> 1
+        k = lo["kbest"][yl, xl]
+        sk = s_lo[k] + lo["delta"][yl, xl] * ((s_lo[k + 1] - s_lo[k]) if lo["delta"][yl, xl] != 0 else 0.0)
+        d_star = 1.0 / sk
+        r = oracle.back_project(cams[0], x, y)
+        X = plane["depth"][y, x] * r                               # the reconstructed point (range along the unit ray)
+        assert abs(n_fam[f_lo[k]] @ X - d_star) < 1e-9 * d_star    # lies on the refined plane of the half-res pixel
+        Xc = copy["depth"][y, x] * r
+        off_plane_copy += abs(n_fam[f_lo[k]] @ Xc - d_star) > 1e-6 * d_star
+        n_checked += 1
+    assert n_checked > 50 and off_plane_copy > 0.5 * n_checked     # the copied ranges do not have that property
+    # the four children of a half-resolution pixel share one plane: their z-depths agree (fronto-parallel family)
+    zmap = oracle.compute_depth_multires(cams, 0, fl, fc, dict(p_lo, **off), dict(p_hi, upsample_plane=1, depth_kind=1, **off), crop, imgs)
+    blocks = 0
+    for yl in range(2, H // 2 - 2, 3):
+        for xl in range(2, W // 2 - 2, 5):
+            blk = (slice(2 * yl, 2 * yl + 2), slice(2 * xl, 2 * xl + 2))
+            if from_lo[blk].all() and (zmap["reason"][blk] == 0).all():
+                assert np.ptp(zmap["depth"][blk]) < 1e-9 * zmap["depth"][blk].max()
+                blocks += 1
+    assert blocks > 20
