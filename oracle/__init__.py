@@ -17,6 +17,7 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "fsw_oracle.c")
+_SRC_TSDF = os.path.join(_HERE, "fsw_tsdf_oracle.c")
 _HDR = os.path.join(_HERE, "fsw_oracle.h")
 _LIB = os.path.join(_HERE, "libfsw_oracle.so")
 _lib = None
@@ -49,11 +50,11 @@ class Params(ctypes.Structure):
 
 
 def build(force: bool = False) -> str:
-    newest = max(os.path.getmtime(_SRC), os.path.getmtime(_HDR))
+    newest = max(os.path.getmtime(_SRC), os.path.getmtime(_SRC_TSDF), os.path.getmtime(_HDR))
     if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < newest:
         tmp = _LIB + ".tmp.%d" % os.getpid()
         subprocess.check_call(["gcc", "-O2", "-std=c11", "-fPIC", "-shared", "-fopenmp", "-ffp-contract=off",
-                               "-Wall", "-o", tmp, _SRC, "-lm"])
+                               "-Wall", "-o", tmp, _SRC, _SRC_TSDF, "-lm"])
         os.replace(tmp, _LIB)
     return _LIB
 
