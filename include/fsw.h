@@ -356,6 +356,64 @@ int32_t fsw_filter_continuity(fsw_context* ctx, const float* depth_in, size_t de
                               float* depth_out, size_t depth_out_pitch, uint8_t* reason_out, size_t reason_pitch,
                               void* cuda_stream);
 
+/* ---- TSDF consumer of the depth maps (section III-C) ------------------------ */
+/* A local map of fixed size around the vehicle (60 m x 60 m x 3 m) as a dense torus of 8^3-voxel blocks on
+ * the device: every voxel holds the running average D(X) of the truncated signed distance (in units of mu, |D| <= 1)
+ * and its observation count w(X) (Eq. 2); every block a state and the number of frames that updated
+ * it.  Readings where the paper is silent are DESIGN.md T1-T6 (blocks of 8^3 voxels, voxel centres at (index + 0.5)
+ * voxel_size, the depth map stores range along the ray and eta is taken against |X_d|, nearest-pixel depth lookup, the
+ * box is snapped to whole blocks).  World coordinates are metres in any fixed frame; poses are world -> camera. */
+typedef struct fsw_tsdf fsw_tsdf;
+
+typedef struct fsw_tsdf_params {
+    uint32_t struct_size;
+    float voxel_size;  /* metres (the paper uses 0.05) */
+    float mu;          /* truncation distance, metres (unstated in the paper; SPEC.md proposes 0.2) */
+    int32_t w_max;     /* cap of the observation count ("capped to a fixed maximum value") */
+    float box_size[3]; /* extent of the local map, metres; rounded up to whole blocks of 8 voxels */
+} fsw_tsdf_params;
+
+typedef struct fsw_tsdf_stats {
+    uint32_t struct_size;
+    int64_t n_new_blocks;     /* blocks allocated by the last fsw_tsdf_integrate */
+    int64_t n_visible_blocks; /* allocated blocks of the local map during the last fsw_tsdf_integrate */
+    int64_t n_voxels_updated; /* voxels that Eq. 2 updated in the last fsw_tsdf_integrate */
+    int64_t n_points;         /* points found by the last fsw_tsdf_extract_points (may exceed its capacity) */
+    int64_t n_blocks_freed;   /* blocks that left the box in the last fsw_tsdf_recentre */
+    int64_t n_frames;         /* depth maps integrated so far */
+} fsw_tsdf_stats;
+
+/* Allocates the local map centred at centre[3] (metres; the box is snapped so that the block that contains the centre
+ * is the middle block).  Errors: FSW_E_INVALID_ARG, FSW_E_CONFIG (more than 2^26 blocks), FSW_E_CUDA, FSW_E_NOMEM.
+ * The TSDF calls keep their own thread-local error text: fsw_tsdf_last_error. */
+int32_t fsw_tsdf_create(int32_t cuda_device, const fsw_tsdf_params* params, const double* centre, fsw_tsdf** out);
+int32_t fsw_tsdf_destroy(fsw_tsdf* vol);
+const char* fsw_tsdf_last_error(void);
+/* integer block coordinate of the box's first block and the number of blocks per axis (host ints, 3 each) */
+int32_t fsw_tsdf_box(const fsw_tsdf* vol, int32_t* block_origin, int32_t* blocks);
+/* Moves the box to a new centre ("we only allocate new voxel blocks within this region and swap old blocks that are
+ * no longer in this region"): blocks whose world coordinate leaves the box are freed (their content is
+ * dropped, nothing is archived), the others keep their content.  Asynchronous on cuda_stream. */
+int32_t fsw_tsdf_recentre(fsw_tsdf* vol, const double* centre, void* cuda_stream);
+/* One depth map: allocation along [d - mu, d + mu] of the Eq. 1 ray of every valid pixel, the list
+ * of the frame's blocks, Eq. 2 for every voxel of those blocks.  cam: intrinsics, distortion and
+ * field of view of the depth camera (its R, t are ignored); R (9, row-major), t (3): world -> camera, X_d = R X + t,
+ * host doubles; depth: DEVICE, float32 [height][width] of that camera, pitch in bytes, range along the pixel ray in
+ * metres, <= 0 = invalid (the maps fsw_compute_depth* writes with FSW_DEPTH_RANGE).  Asynchronous on cuda_stream; the
+ * depth map must stay alive until the stream reaches this work. */
+int32_t fsw_tsdf_integrate(fsw_tsdf* vol, const fsw_camera* cam, const double* R, const double* t, const float* depth,
+                           size_t depth_pitch, void* cuda_stream);
+/* Points of the map: zero crossings of D between axis neighbours that both carry weight, in blocks with at least
+ * min_block_observations updates ("we only consider voxel blocks with at least 3 observations"), placed
+ * by linear interpolation; points: DEVICE, capacity x 3 floats (x, y, z in metres RELATIVE TO THE BOX ORIGIN =
+ * block_origin x 8 x voxel_size), in no particular order; the count is in fsw_tsdf_get_stats. */
+int32_t fsw_tsdf_extract_points(fsw_tsdf* vol, int32_t min_block_observations, float* points, int32_t capacity, void* cuda_stream);
+/* synchronizes the stream of the last TSDF call */
+int32_t fsw_tsdf_get_stats(fsw_tsdf* vol, fsw_tsdf_stats* out);
+/* Dense copy of the local map in box order, for inspection and tests: tsdf / weight DEVICE float32
+ * [blocks_z*8][blocks_y*8][blocks_x*8], observations int32 / allocated uint8 [blocks_z][blocks_y][blocks_x]. */
+int32_t fsw_tsdf_download(fsw_tsdf* vol, float* tsdf, float* weight, int32_t* observations, uint8_t* allocated, void* cuda_stream);
+
 #ifdef __cplusplus
 }
 #endif

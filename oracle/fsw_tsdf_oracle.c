@@ -63,18 +63,18 @@ int64_t orc_tsdf_allocate(const orc_tsdf_box* B, const orc_camera* cam, const do
                 const double range = (d - B->mu) + (double)i * (2.0 * B->mu / (double)n);
                 const double Xd[3] = { range * r[0] - t[0], range * r[1] - t[1], range * r[2] - t[2] };
                 double X[3], f[3];
-                int b[3], near = 0;
+                int b[3], near = 0, side[3] = { 0, 0, 0 }; /* side: the neighbour across a face the sample almost touches */
                 for (int a = 0; a < 3; ++a) { /* X = R^T (X_d - t) */
                     X[a] = R[a] * Xd[0] + R[3 + a] * Xd[1] + R[6 + a] * Xd[2];
                     f[a] = X[a] / edge;
                     b[a] = (int)floor(f[a]);
-                    if (fabs(f[a] - floor(f[a] + 0.5)) < 1e-4) near = 1;
+                    if (fabs(f[a] - floor(f[a] + 0.5)) < 1e-4) { near = 1; side[a] = (f[a] - floor(f[a]) < 0.5) ? -1 : 1; }
                 }
-                if (near && fragile)
-                    for (int dz = -1; dz <= 1; ++dz)
-                        for (int dy = -1; dy <= 1; ++dy)
-                            for (int dx = -1; dx <= 1; ++dx)
-                                if (in_box(B, b[0] + dx, b[1] + dy, b[2] + dz)) fragile[block_slot(B, b[0] + dx, b[1] + dy, b[2] + dz)] = 1;
+                if (near && fragile) /* the sample's block and the blocks across the near face(s) */
+                    for (int m = 0; m < 8; ++m) {
+                        const int dx = (m & 1) ? side[0] : 0, dy = (m & 2) ? side[1] : 0, dz = (m & 4) ? side[2] : 0;
+                        if (in_box(B, b[0] + dx, b[1] + dy, b[2] + dz)) fragile[block_slot(B, b[0] + dx, b[1] + dy, b[2] + dz)] = 1;
+                    }
                 if (!in_box(B, b[0], b[1], b[2])) continue; /* only inside the local map */
                 uint8_t* a = &allocated[block_slot(B, b[0], b[1], b[2])];
                 if (!*a) { *a = 1; ++fresh; }

@@ -40,7 +40,7 @@ def _nvcc() -> str:
 def _sources():
     deps = [os.path.join(CSRC, f) for f in os.listdir(CSRC) if f != os.path.basename(PROBE_SRC)]
     deps += [os.path.join(INCLUDE, "fsw.h"), os.path.abspath(__file__)]
-    units = [("fsw_api.o", "fsw_api.cu", []), ("fsw_aux.o", "fsw_aux.cu", []),
+    units = [("fsw_api.o", "fsw_api.cu", []), ("fsw_aux.o", "fsw_aux.cu", []), ("fsw_tsdf.o", "fsw_tsdf.cu", []),
              ("fsw_sweep_dispatch.o", "fsw_sweep_dispatch.cu", [])]
     # one object per (window, view count): views 1..4 unrolled (3 and 4 only where two views share a pass, i.e. for
     # windows up to 9), 0 = the run-time view loop; the heaviest objects first

@@ -484,7 +484,7 @@ struct SetHot {
  * half-resolution pass as a plane offset d*; the pixel's own ray meets that plane at range d* / (n.r).  Out of line: a
  * rarely used variant must not cost the sweep loop registers.  The ray is recomputed (tiles outside the crop never
  * ran S1).  Returns the depth; sets reason = FSW_REASON_NO_PLANE where the ray does not meet the plane. */
-__device__ __noinline__ float plane_upsampled_depth(const FswSweepArgs& args, int ox, int oy, int kidx, float d_star, int& reason) {
+static __device__ __noinline__ float plane_upsampled_depth(const FswSweepArgs& args, int ox, int oy, int kidx, float d_star, int& reason) {
     int f = 0;
     for (int g = 1; g < args.n_lo_fams; ++g)
         if (kidx >= args.lo_fam_first[g]) f = g;

@@ -32,7 +32,8 @@ def test_library_exports_every_declared_symbol():
     assert len(names) >= 18
     for name in names:
         assert hasattr(lib, name), name
-    assert sorted(binding.EXPORTS) == names
+    from paper_1809_06132_b200.tsdf import TSDF_EXPORTS
+    assert sorted(binding.EXPORTS + TSDF_EXPORTS) == names
     assert fsw.version() == (0, 3)
 
 
@@ -41,6 +42,8 @@ def test_struct_layouts_match_header():
     structs = {"fsw_camera": binding.CCamera, "fsw_plane_family": binding.CFamily, "fsw_rect": binding.CRect,
                "fsw_sweep_params": binding.CParams, "fsw_image": binding.CImage, "fsw_depth_out": binding.CDepthOut,
                "fsw_counters": binding.CCounters}
+    from paper_1809_06132_b200 import tsdf
+    structs.update({"fsw_tsdf_params": tsdf.CTsdfParams, "fsw_tsdf_stats": tsdf.CTsdfStats})
     lines = ['#include <stdio.h>', '#include <stddef.h>', '#include "fsw.h"', 'int main(void){']
     for cname, cls in structs.items():
         lines.append('printf("%s %%zu\\n", sizeof(%s));' % (cname, cname))
