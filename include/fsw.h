@@ -222,8 +222,7 @@ int32_t fsw_planeset_table(const fsw_planeset* ps, double* s, double* d, int32_t
 /* Owns device-side scratch (footprint images of the views, half-resolution images and maps, tile schedule, work
  * queue, counters).  Scratch is allocated lazily and reused, so one context serves one stream at a time.  All work of
  * a call is ordered on the stream given to it: whatever follows the call on that stream sees its results.  The
- * library launches on no other stream ("no hidden streams") unless the caller opts in with
- * fsw_context_set_split(ctx, FSW_SPLIT_AUTO_TWO_STREAMS). */
+ * library launches on no other stream ("no hidden streams"). */
 int32_t fsw_context_create(const fsw_rig* rig, int32_t cuda_device, fsw_context** out);
 int32_t fsw_context_destroy(fsw_context* ctx);
 
@@ -303,26 +302,41 @@ int32_t fsw_compute_depth_multires_batch_host(fsw_context* ctx, const fsw_planes
 int32_t fsw_context_set_host_async(fsw_context* ctx, int32_t on);
 
 /* Load balancing of calls with few frame sets (S0).  The sweep kernel runs one persistent CTA per SM over a queue of
- * (frame set, tile) items; a single 1280 x 1024 frame set has 176 live tiles for 148 SMs.  With the plane split every
- * tile becomes two work items that sweep one half of the planes each (the planes are independent
- * hypotheses) and merge their winner-take-all states; the maps are bit-identical to the unsplit ones.
- * FSW_SPLIT_AUTO (default): when the live tiles of the call are fewer than three per SM, the tiles beyond the last
- * full wave of the grid are split (all of them if there is less than one wave), in ONE launch on the caller's stream;
- * FSW_SPLIT_OFF: never; FSW_SPLIT_ON: every tile.
- * FSW_SPLIT_AUTO_TWO_STREAMS (opt-in, the only mode in which the library uses a stream of its own): as AUTO, but the
- * whole tiles and the halved tiles go into two launches, the second one on a low-priority stream the context creates,
- * forked from and joined to the caller's stream by two events, so that its thread blocks take the SMs the first
- * launch frees (about 5 % less latency for a single 1280 x 1024 frame set).  To the caller the call is still ordered
- * on its stream; under stream capture the fork / join events make the second stream part of the captured graph, but a
- * caller that confines its stream to an SM partition (green context) should not use this mode: the context's stream is
- * created on the device's primary context.
+ * (frame set, tile) items, heaviest first by a host estimate of the work of every tile; a single 1280 x 1024 frame set
+ * has 176 tiles with work for 148 SMs, and its heaviest tile takes longer than the mean load of an SM.  With the plane
+ * split a tile becomes two work items that sweep one half of the planes each (the planes are
+ * independent hypotheses) and merge their winner-take-all states; the maps are bit-identical to the unsplit ones.
+ * FSW_SPLIT_AUTO (default): when the tiles with work are fewer than three per SM, the heavy tiles at the head of the
+ * queue are swept whole and the light ones behind them in halves, how many being chosen to minimise the estimated
+ * makespan.  The two groups are two launches on the caller's stream, the second one a programmatic dependent of the
+ * first (its thread blocks take the SMs the first launch's blocks leave; it completes after the first); no other
+ * stream is involved, and under stream capture the pair is captured like any two launches.
+ * FSW_SPLIT_OFF: never; FSW_SPLIT_ON: every tile in halves, one launch.
  * Calls with fewer than two planes are never split.  The context owns 48 bytes of scratch per reference pixel and
  * frame set of a split call.  Errors: FSW_E_INVALID_ARG for a null context or an unknown mode. */
 #define FSW_SPLIT_AUTO 0
 #define FSW_SPLIT_OFF 1
 #define FSW_SPLIT_ON 2
-#define FSW_SPLIT_AUTO_TWO_STREAMS 3
 int32_t fsw_context_set_split(fsw_context* ctx, int32_t mode);
+
+/* The schedule FSW_SPLIT_AUTO gives a call (S0; host only, no device needed): the queue order of the tiles of the
+ * reference image and how many (tile, frame set) slots at its head are swept whole.  n_blocks: thread blocks of the
+ * persistent grid (the SM count of the device a context would run on).  tile_order / tile_weight (HOST, capacity
+ * entries each, may be NULL with capacity 0): tile index ty * n_tiles_x + tx and estimated work, in plane passes, of
+ * the first min(capacity, n_tiles) tiles of the queue.  The estimate orders the queue and sizes the split; it decides
+ * nothing about the maps.  Errors: FSW_E_INVALID_ARG. */
+typedef struct fsw_schedule_plan {
+    uint32_t struct_size;
+    int32_t tile_w, tile_h;   /* tile size of the window's kernel geometry */
+    int32_t n_tiles_x, n_tiles;
+    int32_t n_live;           /* tiles with work (inside the region of interest and the image circle) */
+    int32_t by_weight;        /* 1: heaviest tile first (short queues); 0: nearest to the principal point first */
+    int64_t n_whole_slots;    /* slots at the head of the queue swept whole; n_tiles * n_sets = no split */
+    int64_t n_halved_slots;   /* the rest: two work items each */
+} fsw_schedule_plan;
+int32_t fsw_plan_schedule(const fsw_rig* rig, const fsw_planeset* planes, const fsw_sweep_params* params, int32_t n_sets,
+                          int32_t n_blocks, int32_t capacity, int32_t* tile_order, float* tile_weight,
+                          fsw_schedule_plan* out);
 
 /* Part of the statistics call below (SURVEY.md 8(b) "stats ... for benches only"): on != 0 makes every following
  * compute call bracket its sweep kernel launches (the dominant kernels, S1-S12) with a pair of CUDA events on the

@@ -6,5 +6,5 @@ The package holds the CUDA sources (csrc/), the in-tree build of libfsw.so (buil
 from .binding import (  # noqa: F401
     DEPTH_RANGE, DEPTH_Z, F32, FILTER_COST, FILTER_RATIO, INDEX_FROM_CROP, INVERSE, LINEAR, REASON_COST_FILTER,
     REASON_MASKED, REASON_NO_PLANE, REASON_OK, REASON_RATIO_FILTER, U8, Context, FswError, PlaneSet, Rig,
-    load_library, version,
+    load_library, plan_schedule, version,
 )

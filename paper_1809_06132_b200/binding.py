@@ -30,6 +30,7 @@ EXPORTS = (
     "fsw_compute_depth_batch", "fsw_compute_depth_batch_host", "fsw_compute_depth_multires_batch",
     "fsw_compute_depth_multires_batch_host", "fsw_rig_subset",
     "fsw_context_set_timing", "fsw_context_set_split", "fsw_context_set_host_async", "fsw_get_last_counters", "fsw_filter_continuity",
+    "fsw_plan_schedule",
 )
 
 
@@ -130,6 +131,7 @@ def load_library():
     L.fsw_context_set_split.argtypes = [vp, i32]
     L.fsw_context_set_host_async.argtypes = [vp, i32]
     L.fsw_get_last_counters.argtypes = [vp, P(CCounters)]
+    L.fsw_plan_schedule.argtypes = [vp, vp, P(CParams), i32, i32, i32, P(i32), P(ctypes.c_float), P(CSchedulePlan)]
     for name in EXPORTS:
         if name != "fsw_last_error":
             getattr(L, name).restype = i32
@@ -171,6 +173,31 @@ def make_family(f) -> CFamily:
     sp = f["spacing"]
     out.spacing = INVERSE if sp in ("inverse", INVERSE) else (LINEAR if sp in ("linear", LINEAR) else int(sp))
     out.d_first, out.d_last = float(f["d_first"]), float(f["d_last"])
+    return out
+
+
+class CSchedulePlan(ctypes.Structure):
+    _fields_ = [("struct_size", ctypes.c_uint32), ("tile_w", ctypes.c_int32), ("tile_h", ctypes.c_int32),
+                ("n_tiles_x", ctypes.c_int32), ("n_tiles", ctypes.c_int32), ("n_live", ctypes.c_int32),
+                ("by_weight", ctypes.c_int32), ("n_whole_slots", ctypes.c_int64), ("n_halved_slots", ctypes.c_int64)]
+
+
+def plan_schedule(rig, planes, params, n_sets=1, n_blocks=148):
+    """fsw_plan_schedule (host only): the queue order of the tiles, their estimated weights and the number of
+    (tile, frame set) slots FSW_SPLIT_AUTO sweeps whole for a call with n_sets frame sets on n_blocks SMs."""
+    import numpy as np
+    L = load_library()
+    cp = make_params(params)
+    plan = CSchedulePlan()
+    plan.struct_size = ctypes.sizeof(CSchedulePlan)
+    _check(L.fsw_plan_schedule(rig.handle, planes.handle, ctypes.byref(cp), n_sets, n_blocks, 0, None, None, ctypes.byref(plan)))
+    order = np.zeros(plan.n_tiles, np.int32)
+    weight = np.zeros(plan.n_tiles, np.float32)
+    _check(L.fsw_plan_schedule(rig.handle, planes.handle, ctypes.byref(cp), n_sets, n_blocks, plan.n_tiles,
+                               order.ctypes.data_as(ctypes.POINTER(ctypes.c_int32)),
+                               weight.ctypes.data_as(ctypes.POINTER(ctypes.c_float)), ctypes.byref(plan)))
+    out = {name: getattr(plan, name) for name, _ in CSchedulePlan._fields_ if name != "struct_size"}
+    out["tile_order"], out["tile_weight"] = order, weight
     return out
 
 
@@ -501,9 +528,8 @@ class Context:
         _check(load_library().fsw_context_set_host_async(self.handle, 1 if on else 0))
 
     def set_split(self, mode="auto"):
-        """fsw_context_set_split: plane split of the tiles of calls with few frame sets ('auto', 'off', 'on', or
-        'auto2' = FSW_SPLIT_AUTO_TWO_STREAMS, the opt-in variant that uses a stream of the context)."""
-        _check(load_library().fsw_context_set_split(self.handle, {"auto": 0, "off": 1, "on": 2, "auto2": 3}[mode]))
+        """fsw_context_set_split: plane split of the light tiles of calls with few frame sets ('auto', 'off', 'on')."""
+        _check(load_library().fsw_context_set_split(self.handle, {"auto": 0, "off": 1, "on": 2}[mode]))
 
     def set_timing(self, on=True):
         """fsw_context_set_timing: bracket the sweep kernels of later calls with CUDA events (last_counters()['sweep_ms'])."""

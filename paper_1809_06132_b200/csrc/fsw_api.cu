@@ -9,6 +9,9 @@
 #include <cstring>
 #include <new>
 #include <algorithm>
+#include <array>
+#include <functional>
+#include <queue>
 #include <vector>
 
 #include "fsw_internal.h"
@@ -95,10 +98,14 @@ struct fsw_planeset {
 
 /* scheduling order of the tiles of one (image size, tile shape, principal point) combination, on the device */
 struct TileOrder {
-    int32_t W, H, tw, th;
-    float cx, cy;
+    uint64_t key;               /* hash of everything the tile weights depend on (tile_order_key) */
     int32_t n_tiles_x, n_tiles;
-    DevBuf dev;
+    int32_t n_live;             /* tiles with work; they come first, heaviest first */
+    std::vector<float> weight;  /* estimated work of the tiles in queue order, in plane passes */
+    std::vector<int32_t> order_w, order_d; /* host copies of the two orders (dev, dev_dist) */
+    std::vector<std::array<int64_t, 3>> whole_for; /* cache of split_whole_for: (n_sets, slots) -> whole slots */
+    DevBuf dev;      /* heaviest first: the order of calls with few frame sets (the split regime) */
+    DevBuf dev_dist; /* nearest to the principal point first: the order of long queues */
 };
 
 /* words of the control block: [0], [1] work queues of the sweep launches, [2..9] four 64-bit counters */
@@ -126,9 +133,6 @@ struct fsw_context {
     DevBuf split_ticket;           /* plane split: one word per (set, tile), zero between launches */
     int32_t split_mode = FSW_SPLIT_AUTO;
     bool host_async = false;       /* the *_host calls return without synchronizing their stream */
-    /* second launch of a split call (the halved tiles), ordered against the caller's stream by two events */
-    cudaStream_t aux_stream = nullptr;
-    cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
     int64_t last_split = 0;        /* sweep launches of the last call that split their tiles */
     std::vector<TileOrder*> orders;
     /* staging for the *_host calls: [set slot] */
@@ -371,35 +375,125 @@ bool view_fov_inside_image(const fsw_camera& c, bool half) {
            (double)d.cy - ry >= 0.5 && (double)d.cy + ry <= (double)d.H - 1.5;
 }
 
-/* Scheduling order of the tiles (S0): nearest to the principal point first, lower image half before the upper
- * half at equal distance (its rays also face ground-parallel planes).  Tiles inside the image circle are the
- * expensive ones; the cheap ones (outside the field of view) fill the tail of the persistent grid. */
-int32_t get_tile_order(fsw_context* ctx, const FswDevCam& ref, const FswSweepGeometry& g, const TileOrder** out) {
+/* FNV-1a over the bytes of the inputs of tile_weights */
+uint64_t tile_order_key(const FswSweepArgs& a, const FswSweepGeometry& g) {
+    uint64_t h = 1469598103934665603ull;
+    auto mix = [&](const void* p, size_t n) {
+        const unsigned char* b = static_cast<const unsigned char*>(p);
+        for (size_t i = 0; i < n; ++i) { h ^= b[i]; h *= 1099511628211ull; }
+    };
+    mix(&a.ref, sizeof(a.ref)); mix(&a.ref_rd2_max, sizeof(float)); mix(&g.tile_w, sizeof(int)); mix(&g.tile_h, sizeof(int));
+    mix(&a.n_fams, sizeof(int)); mix(a.fam, sizeof(FswDevFamily) * (size_t)a.n_fams);
+    mix(&a.n_planes, sizeof(int)); mix(a.inv_d, sizeof(float) * (size_t)a.n_planes);
+    mix(&a.inv_range_max, sizeof(float));
+    const int32_t roi[4] = { a.roi_x0, a.roi_y0, a.roi_x1, a.roi_y1 };
+    mix(roi, sizeof(roi));
+    return h;
+}
+
+/* Estimated work of every tile, in plane passes (host model of what the kernel skips: tiles outside the region of
+ * interest or the image circle, planes no ray of the tile faces or reaches within range_max, rows without rays).
+ * Twelve sample points per tile, rays by the closed-form inverse of the unified model without the distortion: the
+ * figures only order the queue and size the plane split, they decide nothing about the result. */
+void tile_weights(const FswSweepArgs& a, const FswSweepGeometry& g, int hw, int ntx, int nty, std::vector<float>& w) {
+    w.assign((size_t)ntx * nty, 0.f);
+    const FswDevCam& c = a.ref;
+    constexpr int NPX = 4, NPY = 3;
+    for (int ty = 0; ty < nty; ++ty)
+        for (int tx = 0; tx < ntx; ++tx) {
+            const int x0 = tx * g.tile_w, y0 = ty * g.tile_h;
+            if (!(x0 < a.roi_x1 && x0 + g.tile_w > a.roi_x0 && y0 < a.roi_y1 && y0 + g.tile_h > a.roi_y0)) continue;
+            const float nx = std::max(std::max((float)(x0 - hw) - c.cx, c.cx - (float)(x0 + g.tile_w - 1 + hw)), 0.f) / c.fx;
+            const float ny = std::max(std::max((float)(y0 - hw) - c.cy, c.cy - (float)(y0 + g.tile_h - 1 + hw)), 0.f) / c.fy;
+            if (!(nx * nx + ny * ny <= a.ref_rd2_max)) continue; /* the kernel's own test: nothing to do */
+            float ray[NPX * NPY][3];
+            int n_pts = 0;
+            for (int j = 0; j < NPY; ++j)
+                for (int i = 0; i < NPX; ++i) {
+                    const float px = (float)x0 + ((float)i + 0.5f) * (float)g.tile_w / NPX - 0.5f;
+                    const float py = (float)y0 + ((float)j + 0.5f) * (float)g.tile_h / NPY - 0.5f;
+                    if (px < (float)a.roi_x0 || px > (float)(a.roi_x1 - 1) || py < (float)a.roi_y0 || py > (float)(a.roi_y1 - 1)) continue;
+                    const float mx = (px - c.cx) / c.fx, my = (py - c.cy) / c.fy, r2 = mx * mx + my * my;
+                    if (r2 > a.ref_rd2_max) continue;
+                    const float disc = 1.f + (1.f - c.xi * c.xi) * r2;
+                    if (disc < 0.f) continue;
+                    const float zf = (c.xi + std::sqrt(disc)) / (r2 + 1.f);
+                    if (zf - c.xi < c.cos_fov) continue;
+                    ray[n_pts][0] = zf * mx; ray[n_pts][1] = zf * my; ray[n_pts][2] = zf - c.xi;
+                    ++n_pts;
+                }
+            float sum = 0.f;
+            for (int f = 0; f < a.n_fams; ++f) {
+                const FswDevFamily& F = a.fam[f];
+                float q[NPX * NPY];
+                for (int p = 0; p < n_pts; ++p) q[p] = F.n[0] * ray[p][0] + F.n[1] * ray[p][1] + F.n[2] * ray[p][2];
+                for (int k = F.first; k < F.first + F.count; ++k) {
+                    int cnt = 0;
+                    for (int p = 0; p < n_pts; ++p) cnt += (q[p] > FSW_EPS_Q && q[p] * a.inv_d[k] >= a.inv_range_max) ? 1 : 0;
+                    if (cnt) sum += 0.5f + 0.5f * (float)cnt / (float)(NPX * NPY);
+                }
+            }
+            /* S1 and the epilogue are worth about two plane passes; a live tile that sweeps nothing still runs S1 */
+            w[(size_t)ty * ntx + tx] = sum > 0.f ? sum + 2.f : 0.5f;
+        }
+}
+
+/* Scheduling orders of the tiles (S0), tiles without work last in both.  (1) Heaviest first by the estimate of
+ * tile_weights (longest processing time first), nearest to the principal point first among equals: for calls whose
+ * queue is only a wave or two long, where the order decides the makespan (a single 1280 x 1024 frame set: 1.52 ->
+ * 1.48 ms against the other order).  (2) Nearest to the principal point first, lower image half before the upper half
+ * at equal distance: for long queues, where the tail is made of cheap tiles either way and blocks that run together
+ * read neighbouring parts of the views (eight C5 frame sets per launch: 1.150 ms per map against 1.163 with (1)). */
+void plan_tiles(const FswSweepArgs& a, const FswSweepGeometry& g, int hw, TileOrder* t) {
+    const FswDevCam& ref = a.ref;
+    t->key = tile_order_key(a, g);
+    t->n_tiles_x = (ref.W + g.tile_w - 1) / g.tile_w;
+    const int nty = (ref.H + g.tile_h - 1) / g.tile_h;
+    t->n_tiles = t->n_tiles_x * nty;
+    std::vector<float> w;
+    tile_weights(a, g, hw, t->n_tiles_x, nty, w);
+    std::vector<std::pair<std::pair<float, float>, int32_t>> by_w((size_t)t->n_tiles), by_d((size_t)t->n_tiles);
+    for (int ty = 0; ty < nty; ++ty)
+        for (int tx = 0; tx < t->n_tiles_x; ++tx) {
+            const float dx = ((float)tx + 0.5f) * g.tile_w - 0.5f - ref.cx, dy = ((float)ty + 0.5f) * g.tile_h - 0.5f - ref.cy;
+            const float r = std::sqrt(dx * dx + dy * dy);
+            const int32_t id = ty * t->n_tiles_x + tx;
+            by_w[(size_t)id] = std::make_pair(std::make_pair(-w[(size_t)id], r), id);
+            by_d[(size_t)id] = std::make_pair(std::make_pair(w[(size_t)id] > 0.f ? 0.f : 1.f, r - (dy > 0.f ? 0.25f * g.tile_h : 0.f)), id);
+        }
+    std::stable_sort(by_w.begin(), by_w.end());
+    std::stable_sort(by_d.begin(), by_d.end());
+    std::vector<int32_t>& order_w = t->order_w;
+    std::vector<int32_t>& order_d = t->order_d;
+    order_w.resize((size_t)t->n_tiles); order_d.resize((size_t)t->n_tiles);
+    t->weight.resize((size_t)t->n_tiles);
+    t->n_live = 0;
+    for (int i = 0; i < t->n_tiles; ++i) {
+        order_w[(size_t)i] = by_w[(size_t)i].second;
+        order_d[(size_t)i] = by_d[(size_t)i].second;
+        t->weight[(size_t)i] = w[(size_t)order_w[(size_t)i]];
+        if (t->weight[(size_t)i] > 0.f) t->n_live = i + 1;
+    }
+}
+
+int32_t get_tile_order(fsw_context* ctx, const FswSweepArgs& a, const FswSweepGeometry& g, int hw, TileOrder** out) {
+    const uint64_t key = tile_order_key(a, g);
     for (TileOrder* t : ctx->orders)
-        if (t->W == ref.W && t->H == ref.H && t->tw == g.tile_w && t->th == g.tile_h && t->cx == ref.cx && t->cy == ref.cy) {
+        if (t->key == key) {
             *out = t;
             return FSW_OK;
         }
     TileOrder* t = new (std::nothrow) TileOrder;
     if (!t) return fail(FSW_E_NOMEM, "tile order: out of memory");
-    t->W = ref.W; t->H = ref.H; t->tw = g.tile_w; t->th = g.tile_h; t->cx = ref.cx; t->cy = ref.cy;
-    t->n_tiles_x = (ref.W + g.tile_w - 1) / g.tile_w;
-    const int nty = (ref.H + g.tile_h - 1) / g.tile_h;
-    t->n_tiles = t->n_tiles_x * nty;
-    std::vector<std::pair<float, int32_t>> key((size_t)t->n_tiles);
-    for (int ty = 0; ty < nty; ++ty)
-        for (int tx = 0; tx < t->n_tiles_x; ++tx) {
-            float dx = ((float)tx + 0.5f) * g.tile_w - 0.5f - ref.cx, dy = ((float)ty + 0.5f) * g.tile_h - 0.5f - ref.cy;
-            float r = std::sqrt(dx * dx + dy * dy) - (dy > 0.f ? 0.25f * g.tile_h : 0.f);
-            key[(size_t)ty * t->n_tiles_x + tx] = std::make_pair(r, (int32_t)(ty * t->n_tiles_x + tx));
-        }
-    std::stable_sort(key.begin(), key.end());
-    std::vector<int32_t> order((size_t)t->n_tiles);
-    for (int i = 0; i < t->n_tiles; ++i) order[i] = key[i].second;
-    cudaError_t e = t->dev.reserve(sizeof(int32_t) * (size_t)t->n_tiles);
-    if (e == cudaSuccess) e = cudaMemcpy(t->dev.p, order.data(), sizeof(int32_t) * (size_t)t->n_tiles, cudaMemcpyHostToDevice);
+    plan_tiles(a, g, hw, t);
+    const size_t bytes = sizeof(int32_t) * (size_t)t->n_tiles;
+    cudaError_t e = t->dev.reserve(bytes);
+    if (e == cudaSuccess) e = t->dev_dist.reserve(bytes);
+    if (e == cudaSuccess) e = cudaMemcpy(t->dev.p, t->order_w.data(), bytes, cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy(t->dev_dist.p, t->order_d.data(), bytes, cudaMemcpyHostToDevice);
     if (e != cudaSuccess) {
         t->dev.release();
+        t->dev_dist.release();
         delete t;
         return cuda_fail(e, "tile order upload");
     }
@@ -408,111 +502,127 @@ int32_t get_tile_order(fsw_context* ctx, const FswDevCam& ref, const FswSweepGeo
     return FSW_OK;
 }
 
+/* Plane split: how many (tile, set) slots of the queue order are swept whole (by the unsplit kernel) before the
+ * rest goes in halves.  List scheduling of the estimated weights on `slots` blocks, whole tiles first; a half costs
+ * 0.6 of its tile (two halves repeat S1, score the plane across the cut and merge) plus a constant.  The smallest
+ * makespan wins; every tile whole (= no split) is one of the candidates. */
+int64_t split_whole_for(TileOrder* t, int n_sets, long long slots) {
+    for (const auto& c : t->whole_for)
+        if (c[0] == n_sets && c[1] == slots) return c[2];
+    const int n_live = t->n_live;
+    std::vector<double> load((size_t)slots);
+    auto makespan = [&](int n_whole) {
+        std::fill(load.begin(), load.end(), 0.0);
+        std::priority_queue<double, std::vector<double>, std::greater<double>> pq(std::greater<double>(), load);
+        auto put = [&](double w) { double l = pq.top(); pq.pop(); pq.push(l + w); };
+        for (int i = 0; i < n_whole; ++i)
+            for (int s = 0; s < n_sets; ++s) put((double)t->weight[(size_t)i]);
+        for (int i = n_whole; i < n_live; ++i)
+            for (int s = 0; s < 2 * n_sets; ++s) put(0.6 * (double)t->weight[(size_t)i] + 0.5);
+        double m = 0.0;
+        while (!pq.empty()) { m = std::max(m, pq.top()); pq.pop(); }
+        return m;
+    };
+    int best = n_live;
+    double best_m = makespan(n_live);
+    for (int n_whole = n_live - 1; n_whole >= 0; --n_whole) {
+        const double m = makespan(n_whole);
+        if (m < best_m * 0.999) { best_m = m; best = n_whole; }
+    }
+    const int64_t whole = best == n_live ? (int64_t)t->n_tiles * n_sets : (int64_t)best * n_sets;
+    t->whole_for.push_back({ (int64_t)n_sets, (int64_t)slots, whole });
+    return whole;
+}
+
 /* enqueues the sweep kernel for a.n_sets frame sets (a.set0 / a.sets filled by the caller); the queue word must be
  * zero when the kernel starts (the pack launch before it clears it) */
 int32_t launch_sweep(fsw_context* ctx, FswSweepArgs& a, int w, cudaStream_t s) {
     const FswSweepGeometry g = window_geometry(w, a.n_views);
-    const TileOrder* order = nullptr;
-    int32_t rc = get_tile_order(ctx, a.ref, g, &order);
+    TileOrder* order = nullptr;
+    int32_t rc = get_tile_order(ctx, a, g, w / 2, &order);
     if (rc != FSW_OK) return rc;
-    a.tile_order = (const int32_t*)order->dev.p;
+    const long long slots = (long long)ctx->n_sm * g.ctas_per_sm;
+    const bool short_queue = (long long)order->n_live * a.n_sets < 3 * slots;
+    a.tile_order = (const int32_t*)(short_queue ? order->dev.p : order->dev_dist.p);
     a.n_tiles_x = order->n_tiles_x;
     a.n_tiles = order->n_tiles;
     a.queue = ctx->queue();
     a.counters = ctx->counters();
-    const long long slots = (long long)ctx->n_sm * g.ctas_per_sm;
+    const int total_slots = a.n_tiles * a.n_sets;
     /* Plane split (fsw_context_set_split): few frame sets leave the persistent grid unbalanced -- a 1280 x 1024 frame
-     * has 176 live tiles for 148 CTAs, every CTA takes one and 28 take a second one.  Then every tile becomes two
-     * work items with half of the planes (by expected work: a family facing away from the optical axis is reached
-     * by about (1 + n_z)/2 of the rays) and the halves merge their winner-take-all states (fsw_sweep.cuh). */
+     * has 176 tiles with work for 148 CTAs, and the heaviest tile alone takes longer than the mean load of a CTA.
+     * Then the light tiles at the end of the queue become two work items each, with half of the planes (by expected
+     * work: a family facing away from the optical axis is reached by about (1 + n_z)/2 of the rays), and the halves
+     * merge their winner-take-all states (fsw_sweep.cuh).  The heavy tiles at the head of the queue stay whole, in
+     * the unsplit kernel; how many is decided by split_whole_for on the estimated tile weights. */
     a.split = 0;
+    long long split_whole = total_slots;
     if (ctx->split_mode != FSW_SPLIT_OFF && a.n_planes >= 2) {
-        long long live = 0; /* tiles that intersect the region of interest and the image circle (the kernel's test) */
-        const int hw = w / 2;
-        for (int t = 0; t < a.n_tiles; ++t) {
-            const int ty = t / a.n_tiles_x, tx = t - ty * a.n_tiles_x;
-            const int x0 = tx * g.tile_w, y0 = ty * g.tile_h;
-            if (!(x0 < a.roi_x1 && x0 + g.tile_w > a.roi_x0 && y0 < a.roi_y1 && y0 + g.tile_h > a.roi_y0)) continue;
-            const float nx = std::max(std::max((float)(x0 - hw) - a.ref.cx, a.ref.cx - (float)(x0 + g.tile_w - 1 + hw)), 0.f) / a.ref.fx;
-            const float ny = std::max(std::max((float)(y0 - hw) - a.ref.cy, a.ref.cy - (float)(y0 + g.tile_h - 1 + hw)), 0.f) / a.ref.fy;
-            if (nx * nx + ny * ny <= a.ref_rd2_max) ++live;
+        if (ctx->split_mode == FSW_SPLIT_ON) split_whole = 0;
+        else if (short_queue) split_whole = split_whole_for(order, a.n_sets, slots);
+    }
+    if (split_whole < total_slots) {
+        double total = 0.0, acc = 0.0;
+        std::vector<double> wk((size_t)a.n_planes);
+        for (int f = 0; f < a.n_fams; ++f)
+            for (int j = 0; j < a.fam[f].count; ++j) {
+                wk[(size_t)a.fam[f].first + j] = std::max(0.1, 0.5 * (1.0 + (double)a.fam[f].n[2]));
+                total += wk[(size_t)a.fam[f].first + j];
+            }
+        int kb = 1;
+        for (int k = 0; k < a.n_planes - 1; ++k) {
+            acc += wk[(size_t)k];
+            kb = k + 1;
+            if (acc >= 0.5 * total) break;
         }
-        if (ctx->split_mode == FSW_SPLIT_ON || live * a.n_sets < 3 * slots) {
-            double total = 0.0, acc = 0.0;
-            std::vector<double> wk((size_t)a.n_planes);
-            for (int f = 0; f < a.n_fams; ++f)
-                for (int j = 0; j < a.fam[f].count; ++j) {
-                    wk[(size_t)a.fam[f].first + j] = std::max(0.1, 0.5 * (1.0 + (double)a.fam[f].n[2]));
-                    total += wk[(size_t)a.fam[f].first + j];
-                }
-            int kb = 1;
-            for (int k = 0; k < a.n_planes - 1; ++k) {
-                acc += wk[(size_t)k];
-                kb = k + 1;
-                if (acc >= 0.5 * total) break;
-            }
-            int fa = 0, fb = 0;
-            for (int f = 0; f < a.n_fams; ++f) {
-                if (kb - 1 >= a.fam[f].first) fa = f;
-                if (kb >= a.fam[f].first) fb = f;
-            }
-            const size_t mapsz = (size_t)a.ref.W * a.ref.H;
-            FSW_CUDA(ctx->split_state.reserve((size_t)a.n_sets * 2 * 6 * mapsz * sizeof(float)));
-            const size_t tbytes = (size_t)a.n_sets * a.n_tiles * sizeof(unsigned int);
-            if (tbytes > ctx->split_ticket.bytes) {
-                FSW_CUDA(ctx->split_ticket.reserve(tbytes));
-                FSW_CUDA(cudaMemsetAsync(ctx->split_ticket.p, 0, ctx->split_ticket.bytes, s));
-            }
-            a.split = 1;
-            a.split_k = kb;
-            /* As many full waves of whole tiles as the live tiles fill (the heaviest come first in the queue), the
-             * rest in halves: 148 whole + 28 split tiles for one 1280 x 1024 frame set.  FSW_SPLIT_ON halves all. */
-            const long long live_items = live * a.n_sets;
-            a.split_whole = (ctx->split_mode == FSW_SPLIT_ON || live_items < slots) ? 0 : (int32_t)(slots * (live_items / slots));
-            a.split_whole -= a.split_whole % a.n_sets; /* whole tiles of every set: the first launch sees fewer tiles */
-            a.split_adjacent = fa == fb ? 1 : 0;
-            a.split_state = (float*)ctx->split_state.p;
-            a.split_ticket = (unsigned int*)ctx->split_ticket.p;
+        int fa = 0, fb = 0;
+        for (int f = 0; f < a.n_fams; ++f) {
+            if (kb - 1 >= a.fam[f].first) fa = f;
+            if (kb >= a.fam[f].first) fb = f;
         }
+        const size_t mapsz = (size_t)a.ref.W * a.ref.H;
+        FSW_CUDA(ctx->split_state.reserve((size_t)a.n_sets * 2 * 6 * mapsz * sizeof(float)));
+        const size_t tbytes = (size_t)a.n_sets * a.n_tiles * sizeof(unsigned int);
+        if (tbytes > ctx->split_ticket.bytes) {
+            FSW_CUDA(ctx->split_ticket.reserve(tbytes));
+            FSW_CUDA(cudaMemsetAsync(ctx->split_ticket.p, 0, ctx->split_ticket.bytes, s));
+        }
+        a.split = 1;
+        a.split_k = kb;
+        a.split_whole = 0; /* the whole tiles go to the unsplit kernel */
+        a.split_adjacent = fa == fb ? 1 : 0;
+        a.split_state = (float*)ctx->split_state.p;
+        a.split_ticket = (unsigned int*)ctx->split_ticket.p;
     }
     ctx->last_split += a.split;
-    const int total_slots = a.n_tiles * a.n_sets;
-    auto launch_one = [&](const FswSweepArgs& la, cudaStream_t ls) -> cudaError_t {
-        const long long items = la.split ? 2LL * la.slot_count - la.split_whole : (long long)la.n_tiles * la.n_sets;
-        const int grid = (int)(items < slots ? items : slots);
-        const int var = pick_variant(la, la.foot_f16) + (la.split ? 8 : 0);
-        return fsw_launch_sweep(w, la, var, grid, ls);
-    };
+    auto grid_for = [&](long long items) { return (int)(items < slots ? items : slots); };
     a.slot_first = 0;
     a.slot_count = total_slots;
     cudaError_t e;
-    if (a.split && a.split_whole > 0 && ctx->split_mode == FSW_SPLIT_AUTO_TWO_STREAMS) {
-        /* Two launches (opt-in): the whole tiles (the first full waves of the queue) in the unsplit instantiation on the
-         * caller's stream, the halved tiles in the split instantiation on a low-priority stream of the context that
-         * is forked from and joined to the caller's stream by events; its CTAs take the SMs the first launch frees. */
-        if (!ctx->aux_stream) {
-            int lo = 0, hi = 0;
-            FSW_CUDA(cudaDeviceGetStreamPriorityRange(&lo, &hi));
-            FSW_CUDA(cudaStreamCreateWithPriority(&ctx->aux_stream, cudaStreamNonBlocking, lo));
-            FSW_CUDA(cudaEventCreateWithFlags(&ctx->ev_fork, cudaEventDisableTiming));
-            FSW_CUDA(cudaEventCreateWithFlags(&ctx->ev_join, cudaEventDisableTiming));
-        }
+    if (!a.split) {
+        e = fsw_launch_sweep(w, a, pick_variant(a, a.foot_f16), grid_for(total_slots), s);
+    } else if (split_whole == 0) {
+        e = fsw_launch_sweep(w, a, pick_variant(a, a.foot_f16) + 8, grid_for(2LL * total_slots), s);
+    } else {
+        /* Two launches on the caller's stream: the whole tiles in the unsplit instantiation (the split one is about
+         * 15 % slower on a whole tile), then the halved tiles as a PROGRAMMATIC DEPENDENT launch: every block of the
+         * first kernel executes griddepcontrol.launch_dependents when it starts, so the blocks of the second one
+         * become resident as the first one's blocks run out of whole tiles and exit -- the overlap of a second
+         * stream without one.  The two kernels touch disjoint tiles and have a queue word each; a block of the second
+         * kernel waits for the first grid (griddepcontrol.wait) before it exits, so whatever follows in the stream
+         * sees both complete. */
         FswSweepArgs whole = a, halves = a;
-        whole.split = 0; whole.split_whole = 0;
-        whole.n_tiles = a.split_whole / a.n_sets; /* the unsplit kernel sweeps the first n_tiles * n_sets slots */
-        halves.split_whole = 0; halves.slot_first = a.split_whole; halves.slot_count = total_slots - a.split_whole;
+        whole.split = 0;
+        whole.n_tiles = (int32_t)(split_whole / a.n_sets); /* the unsplit kernel sweeps the first n_tiles * n_sets slots */
+        halves.slot_first = (int32_t)split_whole;
+        halves.slot_count = (int32_t)(total_slots - split_whole);
         halves.queue = ctx->queue() + 1;
-        FSW_CUDA(cudaEventRecord(ctx->ev_fork, s));
-        e = launch_one(whole, s);
+        e = fsw_launch_sweep(w, whole, pick_variant(whole, whole.foot_f16), grid_for(split_whole), s);
         if (e == cudaSuccess) {
-            FSW_CUDA(cudaStreamWaitEvent(ctx->aux_stream, ctx->ev_fork, 0));
-            e = launch_one(halves, ctx->aux_stream);
-            FSW_CUDA(cudaEventRecord(ctx->ev_join, ctx->aux_stream));
-            FSW_CUDA(cudaStreamWaitEvent(s, ctx->ev_join, 0));
+            e = fsw_launch_sweep(w, halves, (pick_variant(halves, halves.foot_f16) + 8) | FSW_VARIANT_PROGRAMMATIC,
+                                 grid_for(2LL * halves.slot_count), s);
             ctx->last_launches++;
         }
-    } else {
-        e = launch_one(a, s);
     }
     if (e != cudaSuccess) return cuda_fail(e, "sweep kernel launch");
     ctx->last_launches++;
@@ -805,9 +915,9 @@ int32_t fsw_context_destroy(fsw_context* ctx) {
         if (ctx->sets_ev[i]) cudaEventDestroy(ctx->sets_ev[i]);
     }
     ctx->split_state.release(); ctx->split_ticket.release();
-    if (ctx->aux_stream) { cudaStreamDestroy(ctx->aux_stream); cudaEventDestroy(ctx->ev_fork); cudaEventDestroy(ctx->ev_join); }
     for (TileOrder* t : ctx->orders) {
         t->dev.release();
+        t->dev_dist.release();
         delete t;
     }
     for (int i = 0; i < 4; ++i)
@@ -1165,9 +1275,42 @@ int32_t fsw_context_set_host_async(fsw_context* ctx, int32_t on) {
     return FSW_OK;
 }
 
+int32_t fsw_plan_schedule(const fsw_rig* rig, const fsw_planeset* planes, const fsw_sweep_params* params, int32_t n_sets,
+                          int32_t n_blocks, int32_t capacity, int32_t* tile_order, float* tile_weight,
+                          fsw_schedule_plan* out) {
+    if (!rig || !planes || !out) return fail(FSW_E_INVALID_ARG, "fsw_plan_schedule: null argument");
+    if (out->struct_size != sizeof(fsw_schedule_plan))
+        return fail(FSW_E_INVALID_ARG, "fsw_plan_schedule: struct_size %u != %zu", out->struct_size, sizeof(fsw_schedule_plan));
+    int32_t rc = check_params(params, "params");
+    if (rc != FSW_OK) return rc;
+    if (n_sets < 1 || n_sets > FSW_MAX_BATCH || n_blocks < 1 || capacity < 0 || (capacity > 0 && (!tile_order || !tile_weight)))
+        return fail(FSW_E_INVALID_ARG, "fsw_plan_schedule: n_sets=%d n_blocks=%d capacity=%d", n_sets, n_blocks, capacity);
+    FswSweepArgs a;
+    fill_args(a, *rig, *planes, *params, false);
+    const FswSweepGeometry g = window_geometry(params->window, a.n_views);
+    TileOrder t;
+    plan_tiles(a, g, params->window / 2, &t);
+    const long long slots = (long long)n_blocks * g.ctas_per_sm;
+    const bool short_queue = (long long)t.n_live * n_sets < 3 * slots;
+    out->tile_w = g.tile_w; out->tile_h = g.tile_h;
+    out->n_tiles_x = t.n_tiles_x; out->n_tiles = t.n_tiles; out->n_live = t.n_live;
+    out->by_weight = short_queue ? 1 : 0;
+    const long long total_slots = (long long)t.n_tiles * n_sets;
+    out->n_whole_slots = (short_queue && a.n_planes >= 2) ? split_whole_for(&t, n_sets, slots) : total_slots;
+    out->n_halved_slots = total_slots - out->n_whole_slots;
+    const std::vector<int32_t>& order = short_queue ? t.order_w : t.order_d;
+    std::vector<float> w_by_tile((size_t)t.n_tiles);
+    for (int i = 0; i < t.n_tiles; ++i) w_by_tile[(size_t)t.order_w[(size_t)i]] = t.weight[(size_t)i];
+    for (int i = 0; i < t.n_tiles && i < capacity; ++i) {
+        tile_order[i] = order[(size_t)i];
+        tile_weight[i] = w_by_tile[(size_t)order[(size_t)i]];
+    }
+    return FSW_OK;
+}
+
 int32_t fsw_context_set_split(fsw_context* ctx, int32_t mode) {
     if (!ctx) return fail(FSW_E_INVALID_ARG, "fsw_context_set_split: null context");
-    if (mode != FSW_SPLIT_AUTO && mode != FSW_SPLIT_OFF && mode != FSW_SPLIT_ON && mode != FSW_SPLIT_AUTO_TWO_STREAMS)
+    if (mode != FSW_SPLIT_AUTO && mode != FSW_SPLIT_OFF && mode != FSW_SPLIT_ON)
         return fail(FSW_E_INVALID_ARG, "fsw_context_set_split: mode %d", mode);
     ctx->split_mode = mode;
     return FSW_OK;

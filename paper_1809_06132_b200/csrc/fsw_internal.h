@@ -84,6 +84,8 @@ struct FswSetPtrs {
     uint8_t* out_reason; int64_t out_reason_pitch;
 };
 
+#define FSW_VARIANT_PROGRAMMATIC 0x100 /* flag added to a kernel variant: programmatic dependent launch */
+
 struct FswSweepArgs {
     FswDevCam ref;
     int32_t n_views;

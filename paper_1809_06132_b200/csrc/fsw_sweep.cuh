@@ -381,18 +381,23 @@ struct Wta {
     /* During the sweep the two neighbours of the best live in shared memory (*nbr = (cm, cp), written by this thread
      * only): they change when a new best arrives or the plane after it is scored, which is rare, and ten registers
      * fewer let the sample phase keep more footprint fetches in flight. */
+    /* halo (split tiles only, the iteration after a half's own planes): the plane across the cut is scored only as the
+     * parabola neighbour of a winner next to the cut; with an infinite cost the rest of the state stays as it is, m2
+     * (the lowest cost except the plane next to the cut) included -- selects instead of a branch around the update */
     template <bool KNEXT>
-    __device__ __forceinline__ void update(float c, int k, int dir, bool desc, bool fam_first, float2* __restrict__ nbr) {
+    __device__ __forceinline__ void update(float c_real, int k, int dir, bool desc, bool fam_first, float2* __restrict__ nbr,
+                                           bool halo = false) {
+        const float c = halo ? CUDART_INF_F : c_real;
         /* neighbour of the running best on the far side (same family): not eligible as second best */
         const bool isn = KNEXT ? (k == knext) : (!fam_first && (k == k1 + dir));
         const bool nb = desc ? ((c <= b1) && (c < CUDART_INF_F)) : (c < b1); /* lowest index wins ties */
-        if (isn) nbr->y = c;
+        if (isn) nbr->y = c_real;
         const float t = isn ? s2 : fminf(s2, c);
         s2 = nb ? m2 : t;
         if (nb) *nbr = make_float2(cprev, CUDART_INF_F);
         k1 = nb ? k : k1;
         if (KNEXT) knext = nb ? k + dir : knext;
-        m2 = b1;
+        m2 = halo ? m2 : b1;
         b1 = fminf(b1, c);
         cprev = c;
     }
@@ -558,6 +563,11 @@ __global__ void __launch_bounds__(Geo<WIN>::NT, 1) sweep_kernel(const __grid_con
     const int h_src = h_on ? hrow * G::SB + hrun * RUN : 0;
     float* const h_dst = hs + (h_on ? hrow * G::HS + hrun * RUN : 0);
     const float* const v_src = hs + (grp * RPT) * G::HS + col; /* first row sum of this thread's vertical pass */
+
+    /* An unsplit launch may be followed in the stream by the launch of the halved tiles as its programmatic dependent
+     * (fsw_api.cu: launch_sweep): those blocks take the SMs this grid's blocks leave.  Nothing they read is written
+     * here, so the trigger comes first; they wait for this grid before they exit. */
+    if constexpr (!SPLIT) asm volatile("griddepcontrol.launch_dependents;");
 
     unsigned item = blockIdx.x;
     while (item < (unsigned)n_items) {
@@ -877,12 +887,8 @@ __global__ void __launch_bounds__(Geo<WIN>::NT, 1) sweep_kernel(const __grid_con
                             else if (args.best_k == 2) c = ci >= 2 ? 0.5f * (bk1[i] + bk2[i]) : bk1[i];
                         }
                         c = ci > 0 ? c : CUDART_INF_F;
-                        if (halo) { /* neighbour across the cut of a winner next to it; nothing else changes */
-                            if (st[i].k1 + dir == k) nbr_at(i)->y = c;
-                        } else {
-                            n_eval += ci;
-                            st[i].template update<false>(c, k, dir, desc, it == 0, nbr_at(i));
-                        }
+                        n_eval += halo ? 0 : ci;
+                        st[i].template update<false>(c, k, dir, desc, it == 0, nbr_at(i), halo);
                     }
                     if (dbg) {
                         float* dc = s_set.debug_cost;
@@ -1071,6 +1077,8 @@ __global__ void __launch_bounds__(Geo<WIN>::NT, 1) sweep_kernel(const __grid_con
         __syncthreads();
         item = s_item;
     }
+    /* a dependent launch completes after the grid before it (no-op for a plain launch) */
+    if constexpr (SPLIT) asm volatile("griddepcontrol.wait;" ::: "memory");
 }
 
 /* Kernel variants (fsw_api.cu: pick_variant): projection mode 0..2 (see SweepInst::go) + 3 if the footprints are
@@ -1083,34 +1091,46 @@ struct SweepInst {
     /* MODE 0: any rotation, full distortion polynomial, denominator test; 1: identity rotations, k1-only distortion;
      * 2: any rotation, k1-only distortion (the last two need cos(fov/2) + xi >= 1e-3) */
     template <int MODE, bool F16, bool INSIDE, bool SPLIT>
-    static cudaError_t go(const FswSweepArgs& args, int grid, cudaStream_t stream, bool prepare_only) {
+    static cudaError_t go(const FswSweepArgs& args, int grid, cudaStream_t stream, bool prepare_only, bool programmatic) {
         auto kern = sweep_kernel<WIN, NVT, MODE == 1, MODE == 0, MODE == 0, INSIDE, F16, SPLIT>;
         if (prepare_only) return cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::smem(FUSE));
-        kern<<<grid, G::NT, G::smem(FUSE), stream>>>(args);
-        return cudaGetLastError();
+        if (!programmatic) {
+            kern<<<grid, G::NT, G::smem(FUSE), stream>>>(args);
+            return cudaGetLastError();
+        }
+        /* programmatic dependent launch: the blocks of this grid may become resident as soon as every block of the
+         * kernel before it in the stream has executed griddepcontrol.launch_dependents or exited */
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3((unsigned)grid); cfg.blockDim = dim3(G::NT); cfg.dynamicSmemBytes = G::smem(FUSE); cfg.stream = stream;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        attr[0].val.programmaticStreamSerializationAllowed = 1;
+        cfg.attrs = attr; cfg.numAttrs = 1;
+        return cudaLaunchKernelEx(&cfg, kern, args);
     }
     static constexpr int N_VARIANTS = 16;
     template <bool SPLIT>
-    static cudaError_t dispatch8(const FswSweepArgs& args, int variant, int grid, cudaStream_t stream, bool prep) {
+    static cudaError_t dispatch8(const FswSweepArgs& args, int variant, int grid, cudaStream_t stream, bool prep, bool pdl) {
         switch (variant) {
-            case 0: return go<0, false, false, SPLIT>(args, grid, stream, prep);
-            case 1: return go<1, false, false, SPLIT>(args, grid, stream, prep);
-            case 2: return go<2, false, false, SPLIT>(args, grid, stream, prep);
-            case 3: return go<0, true, false, SPLIT>(args, grid, stream, prep);
-            case 4: return go<1, true, false, SPLIT>(args, grid, stream, prep);
-            case 5: return go<2, true, false, SPLIT>(args, grid, stream, prep);
-            case 6: return go<1, true, true, SPLIT>(args, grid, stream, prep);
-            case 7: return go<2, true, true, SPLIT>(args, grid, stream, prep);
+            case 0: return go<0, false, false, SPLIT>(args, grid, stream, prep, pdl);
+            case 1: return go<1, false, false, SPLIT>(args, grid, stream, prep, pdl);
+            case 2: return go<2, false, false, SPLIT>(args, grid, stream, prep, pdl);
+            case 3: return go<0, true, false, SPLIT>(args, grid, stream, prep, pdl);
+            case 4: return go<1, true, false, SPLIT>(args, grid, stream, prep, pdl);
+            case 5: return go<2, true, false, SPLIT>(args, grid, stream, prep, pdl);
+            case 6: return go<1, true, true, SPLIT>(args, grid, stream, prep, pdl);
+            case 7: return go<2, true, true, SPLIT>(args, grid, stream, prep, pdl);
             default: break;
         }
         return cudaErrorInvalidValue;
     }
-    static cudaError_t dispatch(const FswSweepArgs& args, int variant, int grid, cudaStream_t stream, bool prep) {
-        return variant < 8 ? dispatch8<false>(args, variant, grid, stream, prep)
-                           : dispatch8<true>(args, variant - 8, grid, stream, prep);
+    static cudaError_t dispatch(const FswSweepArgs& args, int variant, int grid, cudaStream_t stream, bool prep, bool pdl = false) {
+        return variant < 8 ? dispatch8<false>(args, variant, grid, stream, prep, pdl)
+                           : dispatch8<true>(args, variant - 8, grid, stream, prep, pdl);
     }
+    /* variant + FSW_VARIANT_PROGRAMMATIC: launched as a programmatic dependent of the kernel before it in the stream */
     static cudaError_t launch(const FswSweepArgs& args, int variant, int grid, cudaStream_t stream) {
-        return dispatch(args, variant, grid, stream, false);
+        return dispatch(args, variant & (FSW_VARIANT_PROGRAMMATIC - 1), grid, stream, false, (variant & FSW_VARIANT_PROGRAMMATIC) != 0);
     }
     static cudaError_t prepare() {
         static const FswSweepArgs dummy = {};

@@ -41,7 +41,7 @@ def test_struct_layouts_match_header():
     """sizeof / offsetof of every ABI struct, as compiled by gcc from include/fsw.h, equal the ctypes mirror."""
     structs = {"fsw_camera": binding.CCamera, "fsw_plane_family": binding.CFamily, "fsw_rect": binding.CRect,
                "fsw_sweep_params": binding.CParams, "fsw_image": binding.CImage, "fsw_depth_out": binding.CDepthOut,
-               "fsw_counters": binding.CCounters}
+               "fsw_counters": binding.CCounters, "fsw_schedule_plan": binding.CSchedulePlan}
     from paper_1809_06132_b200 import tsdf
     structs.update({"fsw_tsdf_params": tsdf.CTsdfParams, "fsw_tsdf_stats": tsdf.CTsdfStats})
     lines = ['#include <stdio.h>', '#include <stddef.h>', '#include "fsw.h"', 'int main(void){']

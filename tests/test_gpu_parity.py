@@ -78,7 +78,8 @@ def test_paper_multiscale_shape_and_its_batch():
     outs = ctx.compute_depth_multires_batch(pl, pc, cfg["params_low"], cfg["params_crop"], cfg["crop"], sets, masks)
     torch.cuda.synchronize()
     c = ctx.last_counters()
-    assert c["n_eval"] == n_eval and c["n_launches"] == 5, c   # downsample, pack + low sweep, pack + crop sweep
+    # downsample, pack + low sweep, pack + crop sweep; a sweep is two launches where the plane split keeps tiles whole
+    assert c["n_eval"] == n_eval and 5 <= c["n_launches"] <= 7, c
     for s in range(2):
         got = oracle.compare.to_numpy(outs[s])
         for key in ("depth", "best_cost", "second_cost", "plane_index", "valid_reason"):
@@ -260,7 +261,8 @@ def test_config4_multires_merge_and_mask():
     k = test["plane_index"].astype(np.int32)
     assert not ((k[outside] >= 0) & ((k[outside] >> 14) & 1).astype(bool)).any()
     assert (test["depth"][mask != 0] == 0).all() and (test["valid_reason"][mask != 0] != 0).all()
-    assert counters["n_launches"] == 5  # downsample, footprint pack + low sweep, footprint pack + crop sweep
+    # downsample, footprint pack + low sweep, footprint pack + crop sweep (two launches each where tiles stay whole)
+    assert 5 <= counters["n_launches"] <= 7
 
 
 @pytest.mark.parametrize("frame", [0, 31])
@@ -290,7 +292,7 @@ def test_config5_batch_of_8_as_benchmarked():
     outs = ctx.compute_depth_batch(planes, cfg["params"], dev_sets, dev_masks)
     torch.cuda.synchronize()
     counters = ctx.last_counters()
-    assert counters["n_launches"] == 2  # one footprint pack, one sweep
+    assert 2 <= counters["n_launches"] <= 3  # one footprint pack, one sweep (two with whole + halved tiles)
     batch = [oracle.compare.to_numpy(o) for o in outs]
     n_eval, n_eval_set = 0, []
     for s in range(8):
@@ -488,7 +490,7 @@ def test_batch_equals_single_calls():
     outs = ctx.compute_depth_batch(planes, p, dev_sets, dev_masks)
     torch.cuda.synchronize()
     c = ctx.last_counters()
-    assert c["n_eval"] == n_eval and c["n_launches"] == 2
+    assert c["n_eval"] == n_eval and 2 <= c["n_launches"] <= 3
     houts = ctx.compute_depth_batch(planes, p, sets, masks, host=True)
     for s in range(5):
         a, b = oracle.compare.to_numpy(outs[s]), oracle.compare.to_numpy(houts[s])
@@ -571,15 +573,15 @@ def test_plane_split_is_bit_identical_to_the_unsplit_sweep():
     planes = fsw.PlaneSet(cfg["families"])
     dev = [torch.from_numpy(im).cuda() for im in synth.render_frame(cfg, 0)]
     res = {}
-    # auto: 148 whole tiles + the other live tiles in halves, one launch; auto2: the same in two launches on two
-    # streams (opt-in); on: every tile in halves
-    for mode in ("off", "auto", "auto2", "on"):
+    # auto: the heavy tiles whole in the unsplit kernel + the light ones in halves as its programmatic dependent launch
+    # (both on the caller's stream); on: every tile in halves, one launch
+    for mode in ("off", "auto", "on"):
         ctx.set_split(mode)
         res[mode] = oracle.compare.to_numpy(ctx.compute_depth(planes, cfg["params"], dev, None))
         c = ctx.last_counters()
         assert c["n_split_launches"] == (0 if mode == "off" else 1)
-        assert c["n_launches"] == (3 if mode == "auto2" else 2), (mode, c)   # pack + sweep(s)
-    for mode in ("auto", "auto2", "on"):
+        assert c["n_launches"] == (3 if mode == "auto" else 2), (mode, c)   # pack + sweep(s)
+    for mode in ("auto", "on"):
         for key in keys:
             assert np.array_equal(res["off"][key], res[mode][key], equal_nan=True), (mode, key)
     ctx.set_split("auto")
@@ -590,9 +592,9 @@ def test_plane_split_is_bit_identical_to_the_unsplit_sweep():
 
 @pytest.mark.parametrize("window", [7, 11])
 def test_plane_split_two_launches_other_windows(window):
-    """An image with more live tiles than SMs and a window other than 9 x 9 (other tile geometry): the automatic modes
-    sweep the first full wave whole and the rest in halves (in one launch, or opt-in in two launches on two streams)
-    and give the unsplit maps bit for bit."""
+    """An image with more live tiles than SMs and a window other than 9 x 9 (other tile geometry): the automatic mode
+    sweeps the heavy tiles whole and the rest in halves (two launches on the caller's stream, the second a programmatic
+    dependent of the first) and gives the unsplit maps bit for bit; so does a back-to-back series of such calls."""
     import torch
     import paper_1809_06132_b200 as fsw
     cfg = _small_rig(W=1216, H=808, n_views=2, fov=170.0)
@@ -601,17 +603,26 @@ def test_plane_split_two_launches_other_windows(window):
     dev = [torch.from_numpy(im).cuda() for im in synth.render_frame(cfg, 0)]
     p = dict(cfg["params"], window=window, filters=3, alpha_upper=0.4, alpha_lower=0.4, beta=1.05, horizon_row=400)
     res = {}
-    for mode in ("off", "auto", "auto2"):
+    for mode in ("off", "auto", "on"):
         ctx.set_split(mode)
         res[mode] = oracle.compare.to_numpy(ctx.compute_depth(planes, p, dev, None))
         c = ctx.last_counters()
-        assert (c["n_split_launches"], c["n_launches"]) == {"off": (0, 2), "auto": (1, 2), "auto2": (1, 3)}[mode], c
+        assert (c["n_split_launches"], c["n_launches"]) == {"off": (0, 2), "auto": (1, 3), "on": (1, 2)}[mode], c
         res[mode + "_n_eval"] = c["n_eval"]
-    assert res["off_n_eval"] == res["auto_n_eval"] == res["auto2_n_eval"] > 0
-    for mode in ("auto", "auto2"):
+    assert res["off_n_eval"] == res["auto_n_eval"] == res["on_n_eval"] > 0
+    for mode in ("auto", "on"):
         for key in ("depth", "best_cost", "second_cost", "plane_index", "valid_reason"):
             assert np.array_equal(res["off"][key], res[mode][key], equal_nan=True), (mode, key)
     assert (res["off"]["plane_index"] >= 0).sum() > 100000
+    # calls issued back to back without a host synchronisation: the pack kernel of a call must not start before both
+    # sweep launches of the call before it are through (the dependent launch completes after the first one)
+    ctx.set_split("auto")
+    outs = [ctx.compute_depth(planes, p, dev, None) for _ in range(6)]
+    torch.cuda.synchronize()
+    for o in outs:
+        o = oracle.compare.to_numpy(o)
+        for key in ("depth", "best_cost", "second_cost", "plane_index", "valid_reason"):
+            assert np.array_equal(res["off"][key], o[key], equal_nan=True), key
     ctx.close()
 
 
