@@ -626,6 +626,37 @@ def test_plane_split_two_launches_other_windows(window):
     ctx.close()
 
 
+def test_split_call_captured_into_a_cuda_graph():
+    """include/fsw.h: the whole / halved launches of FSW_SPLIT_AUTO are two launches on the caller's stream, the second a
+    programmatic dependent of the first; captured into a CUDA graph and replayed they give the maps of the eager call."""
+    import torch
+    import paper_1809_06132_b200 as fsw
+    cfg = synth.make_config(3)
+    _, _, ctx = gpu_objects(cfg)
+    planes = fsw.PlaneSet(cfg["families"])
+    dev = [torch.from_numpy(im).cuda() for im in synth.render_frame(cfg, 0)]
+    keys = ("depth", "best_cost", "second_cost", "plane_index", "valid_reason")
+    eager = ctx.compute_depth(planes, cfg["params"], dev, None)
+    c = ctx.last_counters()
+    assert (c["n_split_launches"], c["n_launches"]) == (1, 3), c
+    eager = {k: eager[k].clone() for k in keys}
+    side = torch.cuda.Stream()
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.stream(side):
+        ctx.compute_depth(planes, cfg["params"], dev, None)     # scratch of the context is allocated outside the capture
+        torch.cuda.synchronize()
+        with torch.cuda.graph(graph, stream=side):
+            out = ctx.compute_depth(planes, cfg["params"], dev, None)
+    for _ in range(3):
+        for k in keys:
+            out[k].zero_()
+        graph.replay()
+        torch.cuda.synchronize()
+        for k in keys:
+            assert np.array_equal(eager[k].cpu().numpy(), out[k].cpu().numpy(), equal_nan=True), k
+    ctx.close()
+
+
 def test_bfloat16_and_float_footprints_agree_bitwise():
     """8-bit views are staged as bfloat16 footprints (exact for integers up to 256), float views as float footprints:
     the same integer-valued views given as uint8 and as float32 must produce bit-identical maps, and a call that
