@@ -57,6 +57,7 @@ extern "C" {
 #define FSW_MAX_FAMILIES 8
 #define FSW_MAX_WINDOW 15
 #define FSW_MAX_BATCH 256 /* frame sets per fsw_compute_depth_batch call */
+#define FSW_STATIC_SCRATCH_BYTES (24u << 20) /* device scratch of fsw_compute_depth_static: 24 MiB per GPU, see there */
 
 /* pixel types of input images */
 #define FSW_U8 0  /* uint8 grey levels 0..255 ("gray scale images") */
@@ -272,6 +273,31 @@ int32_t fsw_compute_depth_multires_batch(fsw_context* ctx, const fsw_planeset* p
                                          fsw_rect crop, int32_t n_sets, const fsw_image* images,
                                          const uint8_t* const* masks, size_t mask_pitch, const fsw_depth_out* outs,
                                          void* cuda_stream);
+
+/* ---- depth for one frame set without any allocation ------------------------- */
+/* fsw_compute_depth (same arguments, same maps bit for bit, steps S1-S12) for callers that may not
+ * allocate device memory: code under CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc.  The
+ * call allocates nothing on the device and nothing pinned (no cudaMalloc, cudaFree, cudaMallocHost): its scratch --
+ * the work-queue word, the tile schedule and the footprint images of the matching views (8 bytes per view pixel for
+ * 8-bit views, 16 for float views) -- lives in one static device array of FSW_STATIC_SCRATCH_BYTES (24 MiB) inside
+ * the library, which every GPU that loads the library holds until the process exits.  The caller passes inputs and
+ * outputs as for fsw_compute_depth (device pointers).
+ * Limit: 256 + 4 x tiles + the footprint images, each rounded up to 256 bytes, must fit the array -- e.g. two 8-bit
+ * views of 1280 x 1024 (21 MB) or four of 1024 x 544 (17.8 MB) do, two float views of 1280 x 1024 do not.  A rig
+ * beyond it gets FSW_E_UNSUPPORTED with the sizes in fsw_last_error() and nothing is launched.
+ * Sharing: there is ONE array per GPU and every call on that GPU uses it, whatever the context or stream.  Calls that
+ * can overlap on the GPU (different streams, or different host threads on different streams) race on it; serialise
+ * them on one stream or with events.  The array keeps the last call's contents: the queue word is cleared by the
+ * call's own first launch, the footprints are rewritten, the tile schedule is re-uploaded only when it changes.
+ * The sweep runs as one launch of the unsplit kernel (the plane split of fsw_context_set_split needs 48 bytes of
+ * state per pixel and is not used), so a single large frame set costs what it costs with FSW_SPLIT_OFF (about a
+ * quarter more than the default at 1280 x 1024).  The context's statistics (fsw_get_last_counters) are not updated.  The first call on a
+ * device resolves the array's device address (cudaGetSymbolAddress) and the first call with a window size sets the
+ * kernels' shared-memory attribute: make one warm-up call before capturing into a graph.  Asynchronous on
+ * cuda_stream.  Errors: as fsw_compute_depth, plus FSW_E_UNSUPPORTED (scratch limit, more than 16384 tiles). */
+int32_t fsw_compute_depth_static(fsw_context* ctx, const fsw_planeset* planes, const fsw_sweep_params* params,
+                                 const fsw_image* images, const uint8_t* mask, size_t mask_pitch,
+                                 const fsw_depth_out* out, void* cuda_stream);
 
 /* Same calls with HOST buffers: images[i].data, mask and every pointer of `out` are host memory (pinned memory
  * makes the copies asynchronous).  The library stages them through context-owned device buffers on cuda_stream:

@@ -21,6 +21,7 @@ FILTER_COST, FILTER_RATIO = 1, 2
 DEPTH_RANGE, DEPTH_Z = 0, 1
 REASON_OK, REASON_NO_PLANE, REASON_COST_FILTER, REASON_RATIO_FILTER, REASON_MASKED = 0, 1, 2, 3, 4
 INDEX_FROM_CROP = 1 << 14
+STATIC_SCRATCH_BYTES = 24 << 20
 
 EXPORTS = (
     "fsw_version", "fsw_last_error", "fsw_rig_create", "fsw_rig_destroy", "fsw_rig_relative_pose",
@@ -30,7 +31,7 @@ EXPORTS = (
     "fsw_compute_depth_batch", "fsw_compute_depth_batch_host", "fsw_compute_depth_multires_batch",
     "fsw_compute_depth_multires_batch_host", "fsw_rig_subset",
     "fsw_context_set_timing", "fsw_context_set_split", "fsw_context_set_host_async", "fsw_get_last_counters", "fsw_filter_continuity",
-    "fsw_plan_schedule",
+    "fsw_plan_schedule", "fsw_compute_depth_static",
 )
 
 
@@ -118,6 +119,7 @@ def load_library():
     multi = [vp, vp, vp, P(CParams), P(CParams), CRect, P(CImage), vp, sz, P(CDepthOut), vp]
     L.fsw_compute_depth.argtypes = single
     L.fsw_compute_depth_host.argtypes = single
+    L.fsw_compute_depth_static.argtypes = single
     L.fsw_compute_depth_multires.argtypes = multi
     batch = [vp, vp, P(CParams), i32, P(CImage), P(vp), sz, P(CDepthOut), vp]
     L.fsw_compute_depth_batch.argtypes = batch
@@ -402,6 +404,23 @@ class Context:
         stream = torch.cuda.current_stream(self.device).cuda_stream
         fn = L.fsw_compute_depth_host if host else L.fsw_compute_depth
         _check(fn(self.handle, planes.handle, ctypes.byref(cp), arr, mptr, mpitch, ctypes.byref(cout), stream))
+        out["_keep"] = (keep, mkeep)
+        return out
+
+    def compute_depth_static(self, planes: PlaneSet, params, images, out, mask=None):
+        """fsw_compute_depth_static: fsw_compute_depth without any device allocation (scratch in the library's static
+        24 MiB array, STATIC_SCRATCH_BYTES).  `out` is required: caller-owned device tensors, so that this wrapper
+        allocates nothing on the device either.  Returns `out`."""
+        torch = _torch()
+        L = load_library()
+        assert out is not None, "compute_depth_static writes into caller-owned tensors"
+        arr, keep = self._images(images, False)
+        mptr, mpitch, mkeep = self._mask(mask, False)
+        cout, out = self._outputs(False, (), out)
+        cp = make_params(params, None)
+        stream = torch.cuda.current_stream(self.device).cuda_stream
+        _check(L.fsw_compute_depth_static(self.handle, planes.handle, ctypes.byref(cp), arr, mptr, mpitch,
+                                          ctypes.byref(cout), stream))
         out["_keep"] = (keep, mkeep)
         return out
 

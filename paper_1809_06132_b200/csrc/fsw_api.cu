@@ -11,6 +11,7 @@
 #include <algorithm>
 #include <array>
 #include <functional>
+#include <mutex>
 #include <queue>
 #include <vector>
 
@@ -1347,6 +1348,156 @@ int32_t fsw_get_last_counters(fsw_context* ctx, fsw_counters* out) {
         if (ctx->n_timed > 1) FSW_CUDA(cudaEventElapsedTime(&t2, ctx->ev[2], ctx->ev[3]));
         out->sweep_ms = (double)t + (double)t2;
     }
+    return FSW_OK;
+}
+
+}  /* extern "C" */
+
+/* ================================================================================================================
+ * fsw_compute_depth_static: the single-frame-set sweep for callers that may not allocate device memory.
+ *
+ * Every byte of device scratch the call needs -- the work-queue word, the tile schedule and the footprint images of
+ * the matching views (S4 staging) -- lives in ONE file-scope array of FSW_STATIC_SCRATCH_BYTES that is part of the
+ * library image: every GPU that loads libfsw.so holds it until the process exits.  In host code the array's name is
+ * only a host-side stand-in for the symbol, not a device address; the address the kernels get comes from
+ * cudaGetSymbolAddress, resolved once per device with that device current (static_scratch_for_device).
+ * ================================================================================================================ */
+static __device__ __align__(256) unsigned char g_fsw_static_scratch[FSW_STATIC_SCRATCH_BYTES];
+
+namespace {
+
+constexpr int FSW_STATIC_MAX_DEVICES = 64;
+constexpr size_t FSW_STATIC_ALIGN = 256;
+constexpr size_t FSW_STATIC_MAX_TILES = 16384; /* tile schedule entries: 64 KiB of the array */
+
+struct StaticScratchDev {
+    unsigned char* base = nullptr; /* device address of g_fsw_static_scratch on this device */
+    bool order_valid = false;      /* the tile schedule now in the array belongs to order_key */
+    uint64_t order_key = 0;
+    bool order_short = false;
+};
+StaticScratchDev g_static_dev[FSW_STATIC_MAX_DEVICES];
+std::mutex g_static_mutex;
+
+size_t align_up(size_t n) { return (n + FSW_STATIC_ALIGN - 1) / FSW_STATIC_ALIGN * FSW_STATIC_ALIGN; }
+
+/* set-up, once per device, `device` current: the device address of the static array */
+int32_t static_scratch_for_device(int device, StaticScratchDev** out) {
+    if (device < 0 || device >= FSW_STATIC_MAX_DEVICES) return fail(FSW_E_UNSUPPORTED, "fsw_compute_depth_static: device %d beyond %d", device, FSW_STATIC_MAX_DEVICES);
+    StaticScratchDev& d = g_static_dev[device];
+    if (!d.base) {
+        unsigned char* p = nullptr;
+        cudaError_t e = cudaGetSymbolAddress((void**)&p, g_fsw_static_scratch);
+        if (e != cudaSuccess) return cuda_fail(e, "fsw_compute_depth_static: cudaGetSymbolAddress of the static scratch array");
+        if (!p || ((uintptr_t)p % FSW_STATIC_ALIGN) != 0) return fail(FSW_E_CUDA, "fsw_compute_depth_static: the static scratch array has no aligned device address");
+        d.base = p;
+    }
+    *out = &d;
+    return FSW_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int32_t fsw_compute_depth_static(fsw_context* ctx, const fsw_planeset* planes, const fsw_sweep_params* params,
+                                 const fsw_image* images, const uint8_t* mask, size_t mask_pitch,
+                                 const fsw_depth_out* out, void* cuda_stream) {
+    const char* who = "fsw_compute_depth_static";
+    if (!ctx || !planes) return fail(FSW_E_INVALID_ARG, "%s: null context or plane set", who);
+    int32_t rc;
+    if ((rc = check_params(params, "params")) != FSW_OK) return rc;
+    if (!images || !out) return fail(FSW_E_INVALID_ARG, "%s: null images or outputs", who);
+    const fsw_rig& rig = ctx->rig;
+    if ((rc = check_images(rig, images)) != FSW_OK) return rc;
+    if ((rc = check_out(rig, out, mask, mask_pitch)) != FSW_OK) return rc;
+
+    /* layout of the array: [0, 256) queue words; the tile schedule; one footprint image per view, each 256-aligned */
+    int f16 = 1;
+    for (int c = 0; c < rig.n_cams; ++c)
+        if (c != rig.ref_index && images[c].dtype != FSW_U8) f16 = 0;
+    FswSweepArgs a;
+    fill_args(a, rig, *planes, *params, false);
+    a.foot_f16 = f16;
+    const FswSweepGeometry g = window_geometry(params->window, a.n_views);
+    const int ntx = (a.ref.W + g.tile_w - 1) / g.tile_w, nty = (a.ref.H + g.tile_h - 1) / g.tile_h;
+    const size_t n_tiles = (size_t)ntx * (size_t)nty;
+    if (n_tiles > FSW_STATIC_MAX_TILES)
+        return fail(FSW_E_UNSUPPORTED, "%s: %zu tiles of %d x %d pixels, the static tile schedule holds %zu", who, n_tiles, g.tile_w, g.tile_h, FSW_STATIC_MAX_TILES);
+    const size_t off_order = FSW_STATIC_ALIGN;
+    size_t need = off_order + align_up(sizeof(int32_t) * n_tiles);
+    size_t off_foot[FSW_MAX_CAMERAS];
+    for (int c = 0; c < rig.n_cams; ++c) {
+        off_foot[c] = need;
+        if (c == rig.ref_index) continue;
+        need += align_up((size_t)rig.cams[c].width * (size_t)rig.cams[c].height * (f16 ? 8u : 16u));
+    }
+    if (need > (size_t)FSW_STATIC_SCRATCH_BYTES)
+        return fail(FSW_E_UNSUPPORTED, "%s: this rig needs %zu bytes of scratch (%d bytes per view pixel), the static array holds %zu: use fsw_compute_depth",
+                    who, need, f16 ? 8 : 16, (size_t)FSW_STATIC_SCRATCH_BYTES);
+
+    cudaStream_t stream = (cudaStream_t)cuda_stream;
+    DeviceGuard dg;
+    FSW_CUDA(dg.enter(ctx->device));
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    StaticScratchDev* sd = nullptr;
+    if ((rc = static_scratch_for_device(ctx->device, &sd)) != FSW_OK) return rc;
+    FSW_CUDA(prepare_window(ctx, params->window)); /* function attributes only */
+    unsigned char* const base = sd->base;
+
+    /* S0: tile schedule.  The array keeps the last call's contents: the schedule is uploaded only when it changes. */
+    const long long slots = (long long)ctx->n_sm * g.ctas_per_sm;
+    const uint64_t key = tile_order_key(a, g);
+    TileOrder plan;
+    plan_tiles(a, g, params->window / 2, &plan);
+    const bool short_queue = (long long)plan.n_live < 3 * slots;
+    if (!sd->order_valid || sd->order_key != key || sd->order_short != short_queue) {
+        sd->order_valid = false;
+        const std::vector<int32_t>& src = short_queue ? plan.order_w : plan.order_d;
+        FSW_CUDA(cudaMemcpyAsync(base + off_order, src.data(), sizeof(int32_t) * n_tiles, cudaMemcpyHostToDevice, stream));
+        sd->order_key = key; sd->order_short = short_queue; sd->order_valid = true;
+    }
+
+    /* S4 staging into the array: one pack launch per view size; the first one clears the queue word */
+    FswSetPtrs set;
+    std::memset(&set, 0, sizeof(set));
+    const fsw_image& ri = images[rig.ref_index];
+    set.ref_img = ri.data; set.ref_pitch_bytes = (int64_t)ri.pitch_bytes; set.ref_dtype = ri.dtype;
+    set.debug_cost = params->debug_cost_volume;
+    set_outputs(set, out, mask, mask_pitch);
+    bool first = true;
+    bool done[FSW_MAX_CAMERAS] = {false};
+    for (int c0 = 0; c0 < rig.n_cams; ++c0) {
+        if (c0 == rig.ref_index || done[c0]) continue;
+        FswPackArgs pk;
+        std::memset(&pk, 0, sizeof(pk));
+        pk.W = rig.cams[c0].width; pk.H = rig.cams[c0].height; pk.f16 = f16;
+        for (int c = c0; c < rig.n_cams; ++c) {
+            if (c == rig.ref_index || done[c] || rig.cams[c].width != pk.W || rig.cams[c].height != pk.H) continue;
+            done[c] = true;
+            const int vi = c < rig.ref_index ? c : c - 1;
+            pk.src[pk.n] = images[c].data; pk.src_pitch[pk.n] = (int64_t)images[c].pitch_bytes; pk.dtype[pk.n] = images[c].dtype;
+            pk.dst[pk.n] = base + off_foot[c];
+            set.foot[vi] = base + off_foot[c];
+            pk.n++;
+        }
+        if (first) { pk.words_to_zero = (unsigned int*)base; pk.n_words_to_zero = FSW_QUEUE_WORDS; first = false; }
+        FSW_CUDA(fsw_launch_pack_footprints(pk, stream));
+    }
+
+    /* the unsplit sweep kernel over every tile (the plane split would need 48 bytes of state per pixel) */
+    a.n_sets = 1;
+    a.set0 = set;
+    a.tile_order = (const int32_t*)(base + off_order);
+    a.n_tiles_x = ntx; a.n_tiles = (int32_t)n_tiles;
+    a.queue = (unsigned int*)base;
+    a.counters = nullptr;
+    a.count_pixels = 0;
+    a.split = 0;
+    a.slot_first = 0; a.slot_count = (int32_t)n_tiles;
+    const long long items = (long long)n_tiles;
+    cudaError_t e = fsw_launch_sweep(params->window, a, pick_variant(a, a.foot_f16), (int)(items < slots ? items : slots), stream);
+    if (e != cudaSuccess) return cuda_fail(e, "sweep kernel launch");
     return FSW_OK;
 }
 

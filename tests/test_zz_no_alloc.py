@@ -1,0 +1,103 @@
+"""-m gpu: fsw_compute_depth_static, the entry point that allocates nothing (scratch in the library's static 24 MiB
+device array, include/fsw.h), against fsw_compute_depth on the same inputs.
+
+The existing tests hold the split and the unsplit sweep of one frame set to bit-identical maps; the static variant runs
+the unsplit kernel over the same tile schedule, so the tolerance here is the same: every map equal bit for bit.  Two
+calls in a row (the array keeps the first call's contents: queue word, tile schedule, footprints), then a different rig
+and a rig beyond the limit.  Collected last (pytest -x must not lose other tests to this one); it
+passes alone in a fresh process and after the other tests.
+"""
+import numpy as np
+import pytest
+
+import synth
+from oracle.compare import to_numpy
+from parity_helpers import gpu_objects
+
+pytestmark = pytest.mark.gpu
+
+MAPS = ("depth", "best_cost", "second_cost", "plane_index", "valid_reason")
+
+
+def _empty_out(torch, H, W, fill):
+    spec = dict(depth=torch.float32, best_cost=torch.float32, second_cost=torch.float32, plane_index=torch.int16,
+                valid_reason=torch.uint8)
+    return {k: torch.full((H, W), fill, dtype=dt, device="cuda:0") for k, dt in spec.items()}
+
+
+def _compare(cfg, frames, mask_seed=None):
+    """the existing path and the static path on every frame of `frames`, the static calls in a row on one stream"""
+    import torch
+    fsw, rig, ctx = gpu_objects(cfg)
+    planes = fsw.PlaneSet(cfg["families"])
+    W, H = rig.sizes[rig.ref_index]
+    mask = None if mask_seed is None else torch.from_numpy(synth.make_mask(W, H, mask_seed)).cuda()
+    sets = [[torch.from_numpy(np.ascontiguousarray(im)).cuda() for im in synth.render_frame(cfg, f)] for f in frames]
+    want = [to_numpy(ctx.compute_depth(planes, cfg["params"], dev, mask)) for dev in sets]
+    torch.cuda.synchronize()
+    outs = [_empty_out(torch, H, W, 7 + i) for i in range(len(sets))]   # allocated before the calls under test
+    before = torch.cuda.memory_allocated(0)
+    free_before = torch.cuda.mem_get_info(0)[0]
+    for dev, out in zip(sets, outs):                                      # two calls in a row, no sync in between
+        ctx.compute_depth_static(planes, cfg["params"], dev, out, mask)
+    torch.cuda.synchronize()
+    assert torch.cuda.memory_allocated(0) == before
+    # nothing was taken from the device outside torch's allocator either (the first call may load the module that
+    # holds the array: the warm-up in the tests below has done that)
+    assert torch.cuda.mem_get_info(0)[0] >= free_before
+    for i, (w, out) in enumerate(zip(want, outs)):
+        got = to_numpy(out)
+        for key in MAPS:
+            assert np.array_equal(w[key], got[key], equal_nan=True), (i, key)
+        assert (got["plane_index"] >= 0).sum() > 0
+    return ctx, planes, sets, outs, want
+
+
+def _warm_up(cfg):
+    """first call on the device: resolves the array's address, sets the kernel attributes (set-up, not under test)"""
+    import torch
+    fsw, rig, ctx = gpu_objects(cfg)
+    W, H = rig.sizes[rig.ref_index]
+    dev = [torch.from_numpy(np.ascontiguousarray(im)).cuda() for im in synth.render_frame(cfg, 0)]
+    ctx.compute_depth_static(fsw.PlaneSet(cfg["families"]), cfg["params"], dev, _empty_out(torch, H, W, 0))
+    torch.cuda.synchronize()
+
+
+def test_static_scratch_matches_the_allocating_path_twice_in_a_row():
+    """BASELINE.json configs[1] (320 x 256 float images: 16-byte footprints, several tiles and a ragged tail), frames 0
+    and 1 back to back, then again in the other order: the second call of each pair finds the first one's queue word,
+    schedule and footprints in the array."""
+    cfg = synth.make_config(2)
+    _warm_up(cfg)
+    _compare(cfg, (0, 1))
+    _compare(cfg, (1, 0))
+
+
+def test_static_scratch_full_size_frame_with_mask_then_a_different_rig():
+    """BASELINE.json configs[2] (two 8-bit views of 1280 x 1024: 21 of the 24 MiB) with a mask, twice in a row; then the
+    small rig of configs[0], whose tile schedule and footprint layout replace the large one's in the same array; then the
+    large one again."""
+    big, small = synth.make_config(3), synth.make_config(1)
+    _warm_up(big)
+    _warm_up(small)
+    _compare(big, (0, 0), mask_seed=11)
+    _compare(small, (0, 0))
+    _compare(big, (0, 0), mask_seed=11)
+
+
+def test_static_scratch_rejects_a_rig_beyond_the_array():
+    """two float views of 1280 x 1024 need 2 x 21 MB: FSW_E_UNSUPPORTED with the sizes in the message, nothing runs"""
+    import torch
+    import paper_1809_06132_b200 as fsw
+    from paper_1809_06132_b200.binding import FswError, STATIC_SCRATCH_BYTES
+    cfg = synth.make_config(3)
+    _, rig, ctx = gpu_objects(cfg)
+    W, H = rig.sizes[rig.ref_index]
+    assert 2 * W * H * 16 > STATIC_SCRATCH_BYTES > 2 * W * H * 8
+    dev = [torch.zeros((H, W), dtype=torch.float32, device="cuda:0") for _ in cfg["cams"]]
+    out = _empty_out(torch, H, W, 3)
+    with pytest.raises(FswError) as err:
+        ctx.compute_depth_static(fsw.PlaneSet(cfg["families"]), cfg["params"], dev, out)
+    assert err.value.code == -5 and "static array holds" in str(err.value)
+    torch.cuda.synchronize()
+    assert float(out["depth"].min()) == 3.0 and float(out["depth"].max()) == 3.0   # untouched
