@@ -73,7 +73,8 @@ extern "C" {
 
 /* depth_kind */
 #define FSW_DEPTH_RANGE 0 /* Euclidean range along the unit ray (PAPER.md:161-162 integrates along the ray) */
-#define FSW_DEPTH_Z 1     /* range * r_z */
+#define FSW_DEPTH_Z 1     /* range * r_z: negative for a ray more than 90 degrees off the optical axis; validity is
+                             valid_reason, not the sign (an invalid pixel holds 0) */
 
 /* reason codes written to fsw_depth_out.valid_reason (0 = valid) */
 #define FSW_REASON_OK 0

@@ -88,7 +88,9 @@ def compare_maps(orc: dict, test: dict, cost_volumes=None, index_flag_mask: int 
     with np.errstate(invalid="ignore", divide="ignore"):
         dc1 = np.abs(np.asarray(test["best_cost"], dtype=np.float64) - orc["c1"])
         dc2 = np.abs(np.asarray(test["second_cost"], dtype=np.float64) - orc["c2"])
-        ddepth = np.abs(np.asarray(test["depth"], dtype=np.float64) - orc["depth"]) / np.maximum(orc["depth"], 1e-30)
+        # relative to |depth|: with FSW_DEPTH_Z (range * r_z, reading Q16) the depth of a ray more than 90 degrees off
+        # the axis is negative; validity is the reason code, not the sign
+        ddepth = np.abs(np.asarray(test["depth"], dtype=np.float64) - orc["depth"]) / np.maximum(np.abs(orc["depth"]), 1e-30)
     cost_set = o_raw & t_raw & (o_k == t_k) & same_source
     depth_set = o_valid & t_valid & (o_k == t_k) & same_source
     max_dc1 = float(dc1[cost_set].max()) if cost_set.any() else 0.0
