@@ -289,7 +289,8 @@ int32_t fsw_compute_depth_multires_batch(fsw_context* ctx, const fsw_planeset* p
  * Sharing: there is ONE array per GPU and every call on that GPU uses it, whatever the context or stream.  Calls that
  * can overlap on the GPU (different streams, or different host threads on different streams) race on it; serialise
  * them on one stream or with events.  The array keeps the last call's contents: the queue word is cleared by the
- * call's own first launch, the footprints are rewritten, the tile schedule is re-uploaded only when it changes.
+ * call's own first launch, the footprints and the tile schedule are rewritten by every call (the schedule by a small
+ * kernel that takes it as launch parameters, not by a copy: a call is kernel launches only).
  * The sweep runs as one launch of the unsplit kernel (the plane split of fsw_context_set_split needs 48 bytes of
  * state per pixel and is not used), so a single large frame set costs what it costs with FSW_SPLIT_OFF (about a
  * quarter more than the default at 1280 x 1024).  The context's statistics (fsw_get_last_counters) are not updated.  The first call on a

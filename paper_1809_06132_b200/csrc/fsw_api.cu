@@ -1364,6 +1364,18 @@ int32_t fsw_get_last_counters(fsw_context* ctx, fsw_counters* out) {
  * ================================================================================================================ */
 static __device__ __align__(256) unsigned char g_fsw_static_scratch[FSW_STATIC_SCRATCH_BYTES];
 
+/* the tile schedule reaches the array through kernel parameters (no copy from pageable host memory, so that even a
+ * call that changes the schedule is a pure sequence of kernel launches); device code of this file names the array
+ * directly */
+struct FswWordChunk {
+    int32_t n, first; /* w[0..n) go to words first .. first + n - 1 of the schedule */
+    int32_t w[960];
+};
+static __global__ void static_schedule_kernel(const __grid_constant__ FswWordChunk c, uint32_t schedule_offset_bytes) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < c.n) reinterpret_cast<int32_t*>(g_fsw_static_scratch + schedule_offset_bytes)[c.first + i] = c.w[i];
+}
+
 namespace {
 
 constexpr int FSW_STATIC_MAX_DEVICES = 64;
@@ -1372,9 +1384,6 @@ constexpr size_t FSW_STATIC_MAX_TILES = 16384; /* tile schedule entries: 64 KiB 
 
 struct StaticScratchDev {
     unsigned char* base = nullptr; /* device address of g_fsw_static_scratch on this device */
-    bool order_valid = false;      /* the tile schedule now in the array belongs to order_key */
-    uint64_t order_key = 0;
-    bool order_short = false;
 };
 StaticScratchDev g_static_dev[FSW_STATIC_MAX_DEVICES];
 std::mutex g_static_mutex;
@@ -1445,17 +1454,22 @@ int32_t fsw_compute_depth_static(fsw_context* ctx, const fsw_planeset* planes, c
     FSW_CUDA(prepare_window(ctx, params->window)); /* function attributes only */
     unsigned char* const base = sd->base;
 
-    /* S0: tile schedule.  The array keeps the last call's contents: the schedule is uploaded only when it changes. */
+    /* S0: tile schedule, written on every call (one small launch): a captured graph that replays an older call may
+     * have put another schedule into the array since, which the host cannot know */
     const long long slots = (long long)ctx->n_sm * g.ctas_per_sm;
-    const uint64_t key = tile_order_key(a, g);
     TileOrder plan;
     plan_tiles(a, g, params->window / 2, &plan);
     const bool short_queue = (long long)plan.n_live < 3 * slots;
-    if (!sd->order_valid || sd->order_key != key || sd->order_short != short_queue) {
-        sd->order_valid = false;
+    {
         const std::vector<int32_t>& src = short_queue ? plan.order_w : plan.order_d;
-        FSW_CUDA(cudaMemcpyAsync(base + off_order, src.data(), sizeof(int32_t) * n_tiles, cudaMemcpyHostToDevice, stream));
-        sd->order_key = key; sd->order_short = short_queue; sd->order_valid = true;
+        FswWordChunk chunk;
+        for (size_t first = 0; first < n_tiles; first += 960) {
+            chunk.n = (int32_t)std::min<size_t>(960, n_tiles - first);
+            chunk.first = (int32_t)first;
+            std::memcpy(chunk.w, src.data() + first, sizeof(int32_t) * (size_t)chunk.n);
+            static_schedule_kernel<<<(chunk.n + 255) / 256, 256, 0, stream>>>(chunk, (uint32_t)off_order);
+            FSW_CUDA(cudaGetLastError());
+        }
     }
 
     /* S4 staging into the array: one pack launch per view size; the first one clears the queue word */

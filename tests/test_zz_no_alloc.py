@@ -122,12 +122,20 @@ def test_static_scratch_call_captured_into_a_cuda_graph():
         torch.cuda.synchronize()
         with torch.cuda.graph(graph, stream=side):
             ctx.compute_depth_static(planes, cfg["params"], dev, out)
-    for _ in range(3):
+    other = synth.make_config(1)            # another rig between the replays: its schedule and footprints take the array
+    _, orig, octx = gpu_objects(other)
+    oW, oH = orig.sizes[orig.ref_index]
+    odev = [torch.from_numpy(np.ascontiguousarray(im)).cuda() for im in synth.render_frame(other, 0)]
+    oplanes, oout = fsw.PlaneSet(other["families"]), _empty_out(torch, oH, oW, 1)
+    for it in range(3):
         for k in MAPS:
             out[k].fill_(9)
         graph.replay()
         torch.cuda.synchronize()
         got = to_numpy(out)
         for k in MAPS:
-            assert np.array_equal(want[k], got[k], equal_nan=True), k
+            assert np.array_equal(want[k], got[k], equal_nan=True), (it, k)
+        octx.compute_depth_static(oplanes, other["params"], odev, oout)
+        torch.cuda.synchronize()
+    octx.close()
     ctx.close()
