@@ -96,9 +96,15 @@ def compare_maps(orc: dict, test: dict, cost_volumes=None, index_flag_mask: int 
     max_dc1 = float(dc1[cost_set].max()) if cost_set.any() else 0.0
     eps_run = min(COST_TOL, max(1.5 * max_dc1, 2e-5))   # the cost error this run shows, not the 1e-4 it is allowed
     if depth_cond is not None:
+        # the bound assumes that the three costs around the minimum carry the run's cost error; on a geometrically
+        # fragile pixel (a window sample within its margin of a view border) a NEIGHBOUR plane may be a mean over
+        # another set of views in one of the two implementations (the same exclusion as for the second best below),
+        # so those pixels only count toward the plain 1e-3 share
+        geom = (orc.get("fragile_geom", np.zeros_like(o_valid, dtype=np.uint8)) != 0)
         allowed = DEPTH_RTOL + 3.0 * eps_run * depth_cond
-        depth_cond_viol = int((ddepth[depth_set] > allowed[depth_set]).sum())
-        worst_ratio = float((ddepth[depth_set] / allowed[depth_set]).max()) if depth_set.any() else 0.0
+        cond_set = depth_set & ~geom
+        depth_cond_viol = int((ddepth[cond_set] > allowed[cond_set]).sum())
+        worst_ratio = float((ddepth[cond_set] / allowed[cond_set]).max()) if cond_set.any() else 0.0
     else:
         depth_cond_viol, worst_ratio = -1, -1.0
     raw_mismatch = (o_raw != t_raw)

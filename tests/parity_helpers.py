@@ -65,7 +65,9 @@ def run_multires(cfg, images, mask, host=False, ctx=None):
     # conditioning of the parabola, taken from whichever pass supplied the pixel
     H, W = ref["depth"].shape
     from_crop = (ref["kbest"] >= 0) & ((ref["kbest"] >> 14) & 1).astype(bool)
-    up = lambda a: np.repeat(np.repeat(a, 2, axis=0), 2, axis=1)[:H, :W]
+    def up(a, fill=0):   # nearest-neighbour upsampling; an odd width / height leaves a last column / row without a source
+        u = np.repeat(np.repeat(a, 2, axis=0), 2, axis=1)[:H, :W]
+        return np.pad(u, ((0, H - u.shape[0]), (0, W - u.shape[1])), constant_values=fill)
     cond_hi = depth_conditioning(ref["hi"], oracle.plane_table(cfg["families_crop"])[0])
     cond_lo = up(depth_conditioning(ref["lo"], oracle.plane_table(cfg["families_low"])[0]))
     cond = np.where(from_crop, cond_hi, cond_lo)

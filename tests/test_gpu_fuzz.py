@@ -105,3 +105,85 @@ def test_random_small_configurations(first):
         assert_gates(st, depth_frac_over_tol=0.05, fragile_frac=0.5, label=label)
     print("fuzz: %d cases with valid pixels, small windows over the 1e-4 cost gate: %s, worst %.2e" % (n_run, json.dumps(over), worst))
     assert n_run >= 20
+
+
+def make_multires_case(seed):
+    """a random two-scale call (fsw_compute_depth_multires): odd and even image sizes, a random crop, either merge order,
+    either upsampling, windows 7..13"""
+    r = np.random.RandomState(seed)
+    W, H = int(r.randint(60, 260)), int(r.randint(50, 190))
+    n_views = int(r.choice([1, 2, 2, 3, 4]))
+    f = float(r.uniform(0.3, 0.7)) * W
+    kw = dict(width=W, height=H, fx=f, fy=f, cx=W / 2.0 + float(r.uniform(-3, 3)), cy=H / 2.0 + float(r.uniform(-3, 3)),
+              xi=float(r.choice([0.6, 0.9, 1.0, 1.3])), fov_max_deg=float(r.choice([140.0, 170.0, 185.0, 200.0])))
+    if r.randint(0, 2):
+        kw.update(k1=float(r.uniform(-0.05, 0.01)))
+    rot = bool(r.randint(0, 2))
+    cams = [synth.camera(**kw)]
+    for _ in range(n_views):
+        c = (float(r.uniform(-0.5, 0.5)), float(r.uniform(-0.3, 0.3)), float(r.uniform(-0.1, 0.1)))
+        if abs(c[0]) + abs(c[1]) < 0.1:
+            c = (0.3, c[1], c[2])
+        cams.append(synth.camera(centre=c, yaw_deg=float(r.uniform(-10, 10)) if rot else 0.0, **kw))
+    dtype = str(r.choice(["u8", "f32"]))
+    vf = synth.VAR_FLOOR_U8 if dtype == "u8" else synth.VAR_FLOOR_F32
+    wl, wc = int(r.choice([7, 9, 9, 11])), int(r.choice([9, 9, 11, 13]))
+    fl = [synth.family((0, 0, 1), int(r.randint(4, 32)), 0.8, 40.0, "inverse")]
+    fc = [synth.family((0, 0, 1), int(r.randint(4, 40)), 0.8, 60.0, "inverse")]
+    if r.randint(0, 2):
+        fl.append(synth.family((0, 1, 0), int(r.randint(2, 8)), 1.1, 2.1, "linear"))
+        fc.append(synth.family((0, 1, 0), int(r.randint(2, 8)), 1.1, 2.1, "linear"))
+    common = dict(alpha_upper=float(r.uniform(0.2, 0.6)), alpha_lower=float(r.uniform(0.2, 0.6)),
+                  beta=float(r.uniform(1.0, 1.3)), subpixel=int(r.randint(0, 2)), filters=int(r.randint(0, 4)),
+                  depth_kind=int(r.randint(0, 2)))
+    hr = int(r.randint(0, H))
+    pl = synth.params(wl, vf, 100.0, horizon_row=hr // 2, **common)
+    pc = synth.params(wc, vf, 120.0, horizon_row=hr, **common)
+    if r.randint(0, 3) == 0:
+        pc["filter_before_merge"] = 1
+    if r.randint(0, 3) == 0:
+        pc["upsample_plane"] = 1
+    x0, y0 = int(r.randint(0, W // 2)), int(r.randint(0, H // 2))
+    crop = (x0, y0, int(r.randint(16, W - x0)), int(r.randint(16, H - y0)))
+    scene = synth.scene_plane(float(r.uniform(2.0, 6.0)), (0.5, 2.0), seed=seed) if r.randint(0, 2) \
+        else synth.scene_boxes(seed=seed, n_boxes=12)
+    cfg = dict(name="mr%d" % seed, dtype=dtype, ref_index=0, cams=cams, families_low=fl, families_crop=fc, params_low=pl,
+               params_crop=pc, crop=crop, scene=scene)
+    mask = synth.make_mask(W, H, seed, n_rects=3) if r.randint(0, 3) == 0 else None
+    return cfg, mask, str(r.choice(["auto", "off", "on"]))
+
+
+@pytest.mark.parametrize("first", [7000, 7030])
+def test_random_multires_configurations(first):
+    from parity_helpers import run_multires
+    n_run, n_odd = 0, 0
+    for seed in range(first, first + 30):
+        cfg, mask, split = make_multires_case(seed)
+        _, _, ctx = gpu_objects(cfg)
+        ctx.set_split(split)
+        images = synth.render_frame(cfg, 0)
+        _, _, stats, _ = run_multires(cfg, images, mask, ctx=ctx)
+        ctx.close()
+        if stats["n_oracle_valid"] == 0:
+            assert stats["valid_mismatch_nonfragile"] == 0 and stats["raw_valid_mismatch_nonfragile"] == 0, (seed, stats)
+            continue
+        n_run += 1
+        n_odd += (cfg["cams"][0]["width"] | cfg["cams"][0]["height"]) & 1
+        pc = cfg["params_crop"]
+        st = dict(stats)
+        if pc["depth_kind"] == 1 and cfg["cams"][0]["fov_max_deg"] > 170.0:   # z-depths near zero, see above
+            st["depth_violations_conditioned"] = 0
+        if min(cfg["params_low"]["window"], pc["window"]) < 9:                # the 7 x 7 half-resolution pass, see above
+            assert st["max_dc1"] <= 1e-3 and st["max_dc2"] <= 1e-3, (seed, st)
+            st["max_dc1"], st["max_dc2"], st["frac_dc2_over_tol"] = min(st["max_dc1"], 1e-4), min(st["max_dc2"], 2e-4), 0.0
+        # with a few hundred valid pixels a handful of flagged pixels (a border sample decides whether the crop pass has a
+        # finite plane at all, i.e. which pass supplies the pixel) is more than 0.1 %: index mismatches that the
+        # flagged validity mismatches account for are excused; valid_mismatch_nonfragile == 0 is still asserted
+        if (1.0 - st["index_match_frac"]) * st["n_oracle_valid"] <= st["valid_mismatch_total"] + 0.5:
+            st["index_match_frac"] = 1.0
+        assert_gates(st, depth_frac_over_tol=0.05, fragile_frac=0.5,
+                     label="multires fuzz seed %d (%dx%d, crop %s, windows %d / %d, %s, split %s)" % (
+                         seed, cfg["cams"][0]["width"], cfg["cams"][0]["height"], cfg["crop"], cfg["params_low"]["window"],
+                         pc["window"], cfg["dtype"], split))
+    print("multires fuzz: %d cases with valid pixels, %d of them with an odd width or height" % (n_run, n_odd))
+    assert n_run >= 10 and n_odd >= 3
