@@ -187,3 +187,66 @@ def test_random_multires_configurations(first):
                          pc["window"], cfg["dtype"], split))
     print("multires fuzz: %d cases with valid pixels, %d of them with an odd width or height" % (n_run, n_odd))
     assert n_run >= 10 and n_odd >= 3
+
+
+@pytest.mark.parametrize("first", [300])
+def test_random_tsdf_integrations(first):
+    """the TSDF consumer (fsw_tsdf_*) on random cameras, poses, voxel sizes, truncation distances and weight caps:
+    allocation equal off the flagged blocks, observation counts exact and D within 1e-4 off the flagged voxels.  The
+    oracle gets the float-rounded voxel size and truncation distance the ABI receives (mu = 0.3 with 0.05 m voxels
+    makes 2 mu / (edge / 2) an integer: with unequal parameter values the two sides take 3 and 4 segment samples)."""
+    import math
+    import torch
+    import oracle.tsdf as OT
+    from paper_1809_06132_b200.tsdf import TsdfVolume
+
+    def yaw(deg):
+        a = math.radians(deg)
+        return np.array([[math.cos(a), 0.0, -math.sin(a)], [0.0, 1.0, 0.0], [math.sin(a), 0.0, math.cos(a)]])
+
+    n_vox = 0
+    for seed in range(first, first + 24):
+        r = np.random.RandomState(seed)
+        W, H = int(r.randint(60, 200)), int(r.randint(50, 150))
+        kw = dict(width=W, height=H, fx=float(r.uniform(0.3, 0.5)) * W, cx=W / 2 + r.uniform(-2, 2),
+                  cy=H / 2 + r.uniform(-2, 2), xi=float(r.choice([0.0, 0.9, 1.0, 1.2])))
+        kw["fy"] = kw["fx"] * float(r.uniform(0.97, 1.03))
+        kw["fov_max_deg"] = float(r.choice([150.0, 170.0, 185.0])) if kw["xi"] > 0.5 else 100.0
+        if r.randint(0, 2):
+            kw["k1"] = float(r.uniform(-0.04, 0.0))
+        cam = synth.camera(**kw)
+        scene = synth.scene_boxes(seed=100 + seed, n_boxes=10)
+        vs, mu = float(np.float32(r.choice([0.05, 0.08, 0.1]))), float(np.float32(r.choice([0.15, 0.2, 0.3])))
+        wmax = int(r.choice([2, 100]))
+        off = r.uniform(0.05, 0.3, 3)
+        frames = []
+        for _ in range(int(r.randint(1, 5))):
+            C, yw = np.array([r.uniform(-0.4, 0.4), r.uniform(-0.1, 0.1), r.uniform(0, 1.0)]), float(r.uniform(-15, 15))
+            c = dict(cam, R=yaw(yw), t=-yaw(yw) @ C)
+            _, rng = synth.render_camera(c, scene, want_range=True)
+            frames.append((dict(c, t=-yaw(yw) @ (C + off)), np.where((rng > 0) & (rng < 10.0), rng, 0.0).astype(np.float32)))
+        centre, size = tuple(np.array([0.0, 0.0, 3.0]) + off), (float(r.choice([6.0, 8.0])), 4.0, float(r.choice([6.0, 8.0])))
+        vol = TsdfVolume(vs, mu, wmax, size, centre)
+        b0, nb = vol.box()
+        assert (b0, nb) == OT.box_for(centre, size, vs), seed
+        ref = OT.Volume(vs, mu, wmax, b0, nb)
+        frag_b, frag_v = np.zeros(ref.allocated.size, np.uint8), np.zeros(ref.D.size, np.uint8)
+        for c, d in frames:
+            vol.integrate(c, c["R"], c["t"], torch.from_numpy(d).cuda())
+            frag_b |= ref.allocate(c, c["R"], c["t"], d, want_fragile=True)[1]
+            frag_v |= ref.integrate(c, c["R"], c["t"], d, want_fragile=True)[1]
+        D, Wt, _, alloc = vol.download()
+        rD, rW, _, ralloc = ref.dense()
+        vol.close()
+        fb3 = frag_b.reshape(alloc.shape) != 0
+        assert not ((alloc != ralloc) & ~fb3).any(), seed
+        up = lambda a: np.repeat(np.repeat(np.repeat(a, 8, axis=0), 8, axis=1), 8, axis=2)
+        nbx, nby, nbz = nb
+        fv3 = frag_v.reshape(nbz, nby, nbx, 8, 8, 8).transpose(0, 3, 1, 4, 2, 5).reshape(D.shape) != 0
+        ok = up((alloc != 0) & (ralloc != 0) & ~fb3) & ~fv3
+        assert np.array_equal(Wt[ok], rW[ok].astype(np.float32)), seed
+        assert np.abs(D[ok] - rD[ok]).max() <= 1e-4, seed
+        assert fv3.mean() < 0.01 and fb3.mean() < 0.1, (seed, fv3.mean(), fb3.mean())
+        n_vox += int(ok.sum())
+    print("tsdf fuzz: %d voxels compared" % n_vox)
+    assert n_vox > 1_000_000

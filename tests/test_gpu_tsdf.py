@@ -17,7 +17,9 @@ import synth
 
 pytestmark = pytest.mark.gpu
 
-VS, MU = 0.05, 0.2
+# the ABI takes voxel size and truncation distance as floats: the oracle gets the same (float-rounded) values, or the
+# number of segment samples n = ceil(2 mu / (edge / 2)) of reading T2 can differ where that ratio is an integer
+VS, MU = float(np.float32(0.05)), float(np.float32(0.2))
 OFFSET = np.array([0.137, 0.093, 0.211])
 
 
