@@ -530,7 +530,14 @@ __global__ void __launch_bounds__(Geo<WIN>::NT, 1) sweep_kernel(const __grid_con
     __shared__ SetHot s_set;
     __shared__ FswDevView s_views[NVT ? 1 : FSW_MAX_VIEWS]; /* run-time view loop: the view parameters */
 
-    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    /* the thread index held in a register (asm volatile): values derived from it are recomputed before their uses
+     * anyway, but from a register and not from S2R */
+    /* (measured: 1.3 % faster at C5 / C3 -- two unrotated views --, 1.2 % slower with four rotated views, 2 % slower
+     * with two rotated ones: kept where it pays) */
+    constexpr bool PIN = (NVT == 1 || NVT == 2) && IDENT;
+    unsigned tid_reg = threadIdx.x;
+    if constexpr (PIN) asm volatile("mov.b32 %0, %0;" : "+r"(tid_reg));
+    const int tid = (int)tid_reg, lane = tid & 31, wid = tid >> 5;
     const int col = tid % TX, grp = tid / TX;
     /* [TY][TX]: reference-side window statistics of every output: ((sum a')/N, sum a'^2 - (sum a')^2/N) */
     float2* const a_stat = reinterpret_cast<float2*>(hs + NJ * 4 * G::HPLANE) + (grp * RPT) * TX + col;
@@ -559,9 +566,27 @@ __global__ void __launch_bounds__(Geo<WIN>::NT, 1) sweep_kernel(const __grid_con
     int hrow_l, hrun;
     h_item<G>(lane, hrow_l, hrun);
     const int hrow = wid * R + hrow_l;
-    const bool h_on = hrow_l >= 0 && hrow < G::EH;
-    const int h_src = h_on ? hrow * G::SB + hrun * RUN : 0;
-    float* const h_dst = hs + (h_on ? hrow * G::HS + hrun * RUN : 0);
+    /* PIN: where the item sits in the sample planes (13 bits) and in the row-sum planes (13 bits), and whether the lane
+     * has one (sign bit), packed into one register that the compiler has to keep: left to itself it recomputes the
+     * three values from the thread index before every use, some 25 instructions per view and pass */
+    static_assert(G::PLANE < 8192 && G::HPLANE < 8192, "13-bit offsets");
+    bool h_on_v;
+    int h_src_v, h_dst_v;
+    if constexpr (PIN) {
+        unsigned hpack = (hrow_l >= 0 && hrow < G::EH)
+                             ? ((unsigned)(hrow * G::SB + hrun * RUN) | ((unsigned)(hrow * G::HS + hrun * RUN) << 13) | 0x80000000u) : 0u;
+        asm volatile("mov.b32 %0, %0;" : "+r"(hpack));
+        h_on_v = (int)hpack < 0;
+        h_src_v = (int)(hpack & 0x1fffu);
+        h_dst_v = (int)((hpack >> 13) & 0x1fffu);
+    } else {
+        h_on_v = hrow_l >= 0 && hrow < G::EH;
+        h_src_v = h_on_v ? hrow * G::SB + hrun * RUN : 0;
+        h_dst_v = h_on_v ? hrow * G::HS + hrun * RUN : 0;
+    }
+    const bool h_on = h_on_v;
+    const int h_src = h_src_v;
+    float* const h_dst = hs + h_dst_v;
     const float* const v_src = hs + (grp * RPT) * G::HS + col; /* first row sum of this thread's vertical pass */
 
     /* An unsplit launch may be followed in the stream by the launch of the halved tiles as its programmatic dependent
