@@ -35,11 +35,11 @@ METRIC = "plane-sweep cost evals/sec (pixel x plane x view)"
 # captures (profiles/), each with the hash of the kernel source it was taken on (kernel_source_hash()): a figure whose
 # hash no longer matches paper_1809_06132_b200/csrc/fsw_sweep.cuh is reported as null, not as a stale number
 NCU_CAPTURES = {
-    ("C5", 8): {"kernel_hash": "40472c9bdaef", "dram_bytes": 156.1e6, "issue_active_pct": 69.9, "fma_pipe_pct": 36.7,
-                "alu_pipe_pct": 37.9, "source": "profiles/r2_sweep_kernel.md (ncu --set full of one 8-set sweep launch)"},
-    ("C3", 8): {"kernel_hash": "40472c9bdaef", "dram_bytes": 153.3e6, "issue_active_pct": 68.9, "fma_pipe_pct": 35.7,
-                "alu_pipe_pct": 37.6, "source": "profiles/r2_sweep_kernel.md (ncu --set full of one 8-set sweep launch)"},
-    ("P", 8): {"kernel_hash": "40472c9bdaef", "dram_bytes": 84.29e6, "issue_active_pct": 66.6, "fma_pipe_pct": 35.3,
+    ("C5", 8): {"kernel_hash": "dd1a26c10355", "dram_bytes": 155.2e6, "issue_active_pct": 68.6, "fma_pipe_pct": 36.2,
+                "alu_pipe_pct": 36.8, "source": "profiles/r2_sweep_kernel.md (ncu --set full of one 8-set sweep launch)"},
+    ("C3", 8): {"kernel_hash": "dd1a26c10355", "dram_bytes": 154.0e6, "issue_active_pct": 67.7, "fma_pipe_pct": 35.3,
+                "alu_pipe_pct": 36.6, "source": "profiles/r2_sweep_kernel.md (ncu --set full of one 8-set sweep launch)"},
+    ("P", 8): {"kernel_hash": "dd1a26c10355", "dram_bytes": 84.7e6, "issue_active_pct": 66.6, "fma_pipe_pct": 35.3,
                "alu_pipe_pct": 38.0, "source": "profiles/r2_sweep_kernel.md (ncu --set full of one 8-set sweep launch)"},
 }
 
